@@ -1,0 +1,133 @@
+/* rlxpp.h -- C ABI of the B200-native RANLUX++ stream library (librlxpp.so).
+ *
+ * Implements the data-parallel hot path of arxiv 2106.02504, Hahnfeld & Moneta,
+ * "A Portable Implementation of RANLUX++".  Citations "P:<n>" are line numbers of
+ * /root/reference/PAPER.md with the section they fall in; "D<k>" / "c-<k>" are the
+ * readings listed in DESIGN.md (the paper prints no algorithm bodies).
+ *
+ * Model.  N independent generator streams.  Stream i holds a 576-bit LCG state X_i
+ * in [0, m), m = 2^576 - 2^240 + 1 (sec. 2.2), and a cursor pos_i in [0, 12]
+ * = number of draws already taken from the block V_i = to_ranlux(X_i) (24 RANLUX
+ * numbers of 24 bits + carry, sec. 2/2.3).  One LCG advance is
+ * X <- A X mod m with A = a^p mod m, p the luxury level;
+ * each advance yields 12 doubles k 2^-48, k = 48 consecutive bits of V.
+ * A fresh stream has pos = 12, i.e. the first draw advances first (D8, c-6).
+ *
+ * Conventions.
+ *   - Every function returns 0 on success and a negative RLXPP_E* code on error;
+ *     rlxpp_last_error() then returns a thread-local, NUL-terminated description.
+ *     No exception crosses the boundary.  There is NO CPU fallback: without a CUDA
+ *     device every compute entry point fails with RLXPP_ECUDA.
+ *   - Pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  The caller
+ *     owns every buffer it passes; the library owns the stream state behind a handle.
+ *   - All work is enqueued on the `cuda_stream` given at creation (a cudaStream_t cast
+ *     to void*, e.g. torch.cuda.current_stream().cuda_stream; NULL = default stream)
+ *     and the calls return WITHOUT synchronising, except the *_host variants, which
+ *     return after the host buffer is complete.
+ *   - 576-bit integers cross the boundary as 9 little-endian uint64_t.
+ */
+#ifndef RLXPP_H
+#define RLXPP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RLXPP_OK 0
+#define RLXPP_EINVAL (-1) /* bad argument (null pointer, n_streams == 0, p == 0, unknown layout ...) */
+#define RLXPP_ECUDA (-2)  /* CUDA runtime error, including "no device" */
+#define RLXPP_ENOMEM (-3) /* device or host allocation failed */
+
+/* output layouts of rlxpp_generate_doubles (BASELINE.json configs 1 and 3) */
+#define RLXPP_STREAM_MAJOR 0 /* out[i * n_per_stream + k] */
+#define RLXPP_INTERLEAVED 1  /* out[k * n_streams + i]   : a warp writes 32 consecutive doubles */
+
+/* state layouts of rlxpp_advance_states */
+#define RLXPP_AOS 0 /* states[i * 9 + limb] */
+#define RLXPP_SOA 1 /* states[limb * n_states + i] */
+
+typedef struct rlxpp rlxpp_t;
+
+/* Creates n_streams streams for luxury level p; stream i is seeded with seed + i
+ * (mod 2^64) by X = (A^(2^96))^(seed + i) mod m, pos = 12 (sec. 2.4
+ * "seed the generator ... fast exponentiation by squaring"; exponent: D7, c-7).
+ * The host computes A = a^p and the square tables; a seeding kernel runs on
+ * `cuda_stream`.  p in {24, 389, 1024, 2048} uses kernels with the multiplier baked
+ * in as immediates; any other p >= 1 uses the generic-multiplier kernels.
+ * Errors: EINVAL (h null, n_streams == 0, p == 0), ENOMEM, ECUDA. */
+int rlxpp_create(rlxpp_t** h, uint64_t n_streams, uint64_t seed, uint32_t p, void* cuda_stream);
+int rlxpp_destroy(rlxpp_t* h);
+
+/* Skips n draws on every stream (rlxpp_skip) or n_dev[i] draws on stream i
+ * (rlxpp_skip_each; n_dev: device pointer, n_streams entries) "without generating
+ * them": X <- A^k X, k = floor((pos + n - 1) / 12), pos <- pos + n - 12 k
+ * (D8, c-8).  Full 64-bit range; n == 0 is a no-op. */
+int rlxpp_skip(rlxpp_t* h, uint64_t n);
+int rlxpp_skip_each(rlxpp_t* h, const uint64_t* n_dev);
+
+/* Handle-free raw LCG arithmetic (BASELINE.json configs[1]): every uint64[9] value
+ * x in [0, 2^576) (non-canonical values >= m allowed) is replaced, in place, by
+ * A^reps x mod m, A = a^p, canonical (< m "in all cases").  multiply9x9
+ * + mod_m per repetition.  reps == 0 only canonicalises.
+ * states_dev: device pointer, 9 * n_states uint64_t, 16-byte aligned, `layout`
+ * RLXPP_AOS or RLXPP_SOA.  n_states == 0 is a no-op. */
+int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, uint32_t reps, int layout,
+                         void* cuda_stream);
+
+/* The next n_per_stream draws of every stream as doubles in [0, 1) on the 2^-48
+ * lattice ("uses only 48 bits for each floating point value"; P:174 one LCG
+ * operation per 12 numbers), written to out_dev (>= n_streams * n_per_stream doubles,
+ * 16-byte aligned) in `layout`.  Any n_per_stream >= 0; multiples of 12 on streams
+ * whose cursors are all at 12 take the fast path.  The streams' states advance. */
+int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout);
+
+/* Same draws, consumed in registers (sec. 4.2: "we sum all numbers per thread
+ * and store them into global memory at the end"): per stream, in draw order,
+ * S <- S + d and Q <- fma(d, d, Q) in IEEE fp64 round-to-nearest, both from +0.0
+ * (c-14).  sum_dev / sumsq_dev: n_streams doubles each (sumsq_dev may be NULL). */
+int rlxpp_generate_reduce(rlxpp_t* h, double* sum_dev, double* sumsq_dev, uint64_t n_per_stream);
+
+/* End-to-end variants with HOST destination buffers: generation on the device in
+ * chunks of streams, device->host copies overlapped on a second CUDA stream; they
+ * return when out_host is complete.  Pinned host memory gives full PCIe rate. */
+int rlxpp_generate_doubles_host(rlxpp_t* h, double* out_host, uint64_t n_per_stream, int layout);
+int rlxpp_generate_reduce_host(rlxpp_t* h, double* sum_host, double* sumsq_host, uint64_t n_per_stream);
+
+/* Exports the paper's stored state (24 RANLUX numbers packed in uint64[9] + carry)
+ * and the cursor; optionally also the LCG form.  Any pointer may be NULL.
+ * ranlux_dev, lcg_dev: [n_streams][9] uint64_t;  carry_dev, pos_dev: [n_streams] uint32_t. */
+int rlxpp_get_state(rlxpp_t* h, uint64_t* ranlux_dev, uint32_t* carry_dev, uint32_t* pos_dev, uint64_t* lcg_dev);
+
+/* Imports states (sec. 4.2: "the state can be copied between host and device"):
+ * lcg_dev [n_streams][9] canonical LCG states (values >= m are reduced), pos_dev
+ * [n_streams] cursors in [0, 12] (NULL = all 12).  Errors: EINVAL. */
+int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev);
+
+/* Host-only helpers: A = a^p mod m as computed by the library's own host arithmetic,
+ * and the seed state (A^(2^96))^seed mod m.  out: 9 uint64_t on the host. */
+int rlxpp_multiplier(uint32_t p, uint64_t* out_host);
+int rlxpp_seed_state(uint64_t seed, uint32_t p, uint64_t* out_host);
+
+uint64_t rlxpp_n_streams(const rlxpp_t* h);
+/* 1 if the kernels with immediate multipliers serve this luxury level */
+int rlxpp_has_fixed_multiplier(uint32_t p);
+/* number of kernel launches this library has enqueued in this process (bench.py's gpu_launches) */
+uint64_t rlxpp_launch_count(void);
+
+/* Roofline denominators measured on the device the caller is on:
+ *   imad: a dependency-free stream of IMAD.WIDE.U32.X (carry-chained, 64-bit accumulate)
+ *         issued from every SM; returns multiply-accumulates per second.
+ *   hbm_write: a write-only kernel storing `bytes` bytes with 128-bit stores; bytes/s.
+ * Both time `iters` launches with CUDA events after a warm-up and report the best. */
+int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream);
+int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s, void* cuda_stream);
+
+const char* rlxpp_last_error(void);
+const char* rlxpp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RLXPP_H */

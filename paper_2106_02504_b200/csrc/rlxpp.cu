@@ -1,0 +1,880 @@
+// librlxpp: RANLUX++ stream generation for B200 (sm_100a).  C ABI in include/rlxpp.h.
+//
+// Hot path: one thread per stream, the 576-bit state as 18 x 32-bit
+// limbs in registers.  Per LCG advance:
+//   multiply9x9  -> 324 IMAD.WIDE.U32.X with the fixed multiplier as immediates, rows
+//                   pre-reduced mod m (rows_generated.cuh)
+//   mod_m        -> fold of the top 37 bits (fold_fast; exact fallback mod_m20)
+//   to_ranlux    -> 8-limb add + carry decision (to_ranlux_fast; exact fallback)
+//   12 doubles   -> byte permutes + one exact DADD each; coalesced 64-bit stores
+//                   (interleaved layout), 128-bit stores (stream-major) or DADD/DFMA
+//                   accumulation in registers (fused reduce).
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/rlxpp.h"
+#include "arith.cuh"
+#include "host_bigint.h"
+#include "rows_generated.cuh"
+
+namespace rlx {
+
+// ----------------------------------------------------------------------------- errors
+static thread_local std::string g_last_error;
+static std::atomic<uint64_t> g_launches{0};
+
+static int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_last_error = buf;
+  return code;
+}
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t _e = (expr);                                                                   \
+    if (_e != cudaSuccess)                                                                     \
+      return fail(_e == cudaErrorMemoryAllocation ? RLXPP_ENOMEM : RLXPP_ECUDA, "%s: %s", #expr, \
+                  cudaGetErrorString(_e));                                                     \
+  } while (0)
+#define LAUNCH_CHECK()        \
+  do {                        \
+    g_launches++;             \
+    CUDA_TRY(cudaGetLastError()); \
+  } while (0)
+
+constexpr int kThreads = 128;
+
+// ----------------------------------------------------------------------------- state I/O
+// Stream state in HBM: 5 planes of uint4, plane g holds limbs 4g .. 4g+3 of every stream
+// (plane 4: limbs 16, 17, pos, 0).  Thread i reads st[g * n + i]: a warp moves 512 contiguous
+// bytes per 128-bit access.  80 B per stream.
+__device__ __forceinline__ void load_state(const uint4* __restrict__ st, u64 n, u64 i, u32 (&x)[18], u32& pos) {
+#pragma unroll
+  for (int g = 0; g < 4; g++) {
+    const uint4 q = st[(u64)g * n + i];
+    x[4 * g] = q.x; x[4 * g + 1] = q.y; x[4 * g + 2] = q.z; x[4 * g + 3] = q.w;
+  }
+  const uint4 q = st[4 * n + i];
+  x[16] = q.x; x[17] = q.y; pos = q.z;
+}
+__device__ __forceinline__ void store_state(uint4* __restrict__ st, u64 n, u64 i, const u32 (&x)[18], u32 pos) {
+#pragma unroll
+  for (int g = 0; g < 4; g++) st[(u64)g * n + i] = make_uint4(x[4 * g], x[4 * g + 1], x[4 * g + 2], x[4 * g + 3]);
+  st[4 * n + i] = make_uint4(x[16], x[17], pos, 0u);
+}
+
+struct Limbs18 { u32 v[18]; };
+
+// ----------------------------------------------------------------------------- slow paths
+// Exact recomputation from the unreduced 20-limb product; reached with probability ~2^-16
+// per advance (carry out of the 8-limb addition in to_ranlux_fast), far less for the rest.
+__device__ __noinline__ void exact_fold(const u32* zin, u32* xout) {
+  u32 z[20], x[18];
+#pragma unroll
+  for (int j = 0; j < 20; j++) z[j] = zin[j];
+  mod_m20(z, x);
+#pragma unroll
+  for (int j = 0; j < 18; j++) xout[j] = x[j];
+}
+__device__ __noinline__ void exact_fold_to_ranlux(const u32* zin, u32* xout, u32* vout, u32* cout) {
+  u32 z[20], x[18], v[18], c;
+#pragma unroll
+  for (int j = 0; j < 20; j++) z[j] = zin[j];
+  mod_m20(z, x);
+  to_ranlux_exact(x, v, c);
+#pragma unroll
+  for (int j = 0; j < 18; j++) { xout[j] = x[j]; vout[j] = v[j]; }
+  *cout = c;
+}
+
+// ----------------------------------------------------------------------------- advance
+// Multiplier policy: Fixed<P> bakes A = a^P into the instruction stream; Generic carries A
+// as 18 runtime limbs (kernel parameter -> uniform registers) and runs the full-width
+// multiply9x9 + mod_m.
+template <int P>
+struct Fixed {
+  static constexpr bool kFixed = true;
+  __device__ __forceinline__ Fixed(const Limbs18&) {}
+  // x <- A x mod m (canonical)
+  __device__ __forceinline__ void advance(u32 (&x)[18]) const {
+    u64 E[9], O[9];
+    u32 e9, o9, z[20], rare = 0;
+    FixedMultiplier<P>::mul(x, E, e9, O, o9);
+    merge_eo(E, e9, O, o9, z);
+    fold_fast(z, x, rare);
+    if (__builtin_expect(rare != 0, 0)) exact_fold(z, x);
+  }
+  // x <- A x mod m and v, c <- to_ranlux(x)
+  __device__ __forceinline__ void advance_block(u32 (&x)[18], u32 (&v)[18], u32& c) const {
+    u64 E[9], O[9];
+    u32 e9, o9, z[20], rare = 0;
+    FixedMultiplier<P>::mul(x, E, e9, O, o9);
+    merge_eo(E, e9, O, o9, z);
+    fold_fast(z, x, rare);
+    to_ranlux_fast(x, v, c, rare);
+    if (__builtin_expect(rare != 0, 0)) exact_fold_to_ranlux(z, x, v, &c);
+  }
+};
+struct Generic {
+  static constexpr bool kFixed = false;
+  u32 a[18];
+  __device__ __forceinline__ Generic(const Limbs18& A) {
+#pragma unroll
+    for (int j = 0; j < 18; j++) a[j] = A.v[j];
+  }
+  __device__ __forceinline__ void advance(u32 (&x)[18]) const {
+    u32 r[18];
+    mulmod_generic(x, a, r);
+#pragma unroll
+    for (int j = 0; j < 18; j++) x[j] = r[j];
+  }
+  __device__ __forceinline__ void advance_block(u32 (&x)[18], u32 (&v)[18], u32& c) const {
+    advance(x);
+    to_ranlux_exact(x, v, c);
+  }
+};
+
+// ----------------------------------------------------------------------------- kernels
+// cfg2: x <- A^reps x mod m on raw uint64[9] states, in place.
+template <class Mult, int LAYOUT>
+__global__ void __launch_bounds__(kThreads) advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
+                                                                  const __grid_constant__ Limbs18 A) {
+  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kThreads * 72 / 16 : 1];
+  const u64 base = (u64)blockIdx.x * kThreads;
+  const u64 i = base + threadIdx.x;
+  u32 x[18];
+  if (LAYOUT == RLXPP_AOS) {
+    // the block's 128 states are 9216 contiguous bytes: 128-bit coalesced loads into shared
+    // memory, then each thread picks up its 72 bytes (stride 18 words: 2-way bank conflict)
+    const u64 cnt = (n - base < (u64)kThreads ? n - base : (u64)kThreads) * 72 / 8;  // u64 words
+    const uint4* src = reinterpret_cast<const uint4*>(states + base * 9);
+    for (u32 q = threadIdx.x; q < (cnt + 1) / 2; q += kThreads) {
+      if (2 * (u64)q + 1 < cnt) stage[q] = src[q];
+      else {  // odd tail: last 8 bytes
+        const u64 lastw = states[base * 9 + 2 * (u64)q];
+        stage[q] = make_uint4((u32)lastw, (u32)(lastw >> 32), 0u, 0u);
+      }
+    }
+    __syncthreads();
+    const u32* sw = reinterpret_cast<const u32*>(stage);
+    if (i < n) {
+#pragma unroll
+      for (int j = 0; j < 18; j++) x[j] = sw[threadIdx.x * 18 + j];
+    }
+  } else {
+    if (i < n) {
+#pragma unroll
+      for (int l = 0; l < 9; l++) {
+        const u64 w = states[(u64)l * n + i];
+        x[2 * l] = (u32)w;
+        x[2 * l + 1] = (u32)(w >> 32);
+      }
+    }
+  }
+  if (i < n) {
+    const Mult mult(A);
+    if (reps == 0) {
+      u32 z[20], r[18];
+#pragma unroll
+      for (int j = 0; j < 20; j++) z[j] = j < 18 ? x[j] : 0u;
+      exact_fold(z, r);
+#pragma unroll
+      for (int j = 0; j < 18; j++) x[j] = r[j];
+    }
+#pragma unroll 1
+    for (u32 r = 0; r < reps; r++) mult.advance(x);
+  }
+  if (LAYOUT == RLXPP_AOS) {
+    __syncthreads();
+    u32* sw = reinterpret_cast<u32*>(stage);
+    if (i < n) {
+#pragma unroll
+      for (int j = 0; j < 18; j++) sw[threadIdx.x * 18 + j] = x[j];
+    }
+    __syncthreads();
+    const u64 cnt = (n - base < (u64)kThreads ? n - base : (u64)kThreads) * 72 / 8;
+    uint4* dst = reinterpret_cast<uint4*>(states + base * 9);
+    for (u32 q = threadIdx.x; q < (cnt + 1) / 2; q += kThreads) {
+      if (2 * (u64)q + 1 < cnt) dst[q] = stage[q];
+      else states[base * 9 + 2 * (u64)q] = (u64)stage[q].x | ((u64)stage[q].y << 32);
+    }
+  } else if (i < n) {
+#pragma unroll
+    for (int l = 0; l < 9; l++) states[(u64)l * n + i] = (u64)x[2 * l] | ((u64)x[2 * l + 1] << 32);
+  }
+}
+
+struct GenArgs {
+  uint4* st;     // state planes of the whole handle
+  u64 n_total;   // streams in the handle (plane stride)
+  u64 first;     // first stream of this launch
+  u64 count;     // streams in this launch
+  double* out;   // output of this launch (already offset to its first stream)
+  u64 ld;        // INTERLEAVED: doubles between consecutive draws of one stream
+  u64 n_per;     // draws per stream
+  double* sum;   // REDUCE: per-stream outputs of this launch (already offset)
+  double* sumsq;
+  Limbs18 A;
+};
+
+enum { kStoreStreamMajor = 0, kStoreInterleaved = 1, kReduce = 2 };
+
+template <int MODE>
+struct Sink {
+  double* p;      // STREAM_MAJOR: &out[i_local * n_per]; INTERLEAVED: &out[i_local]
+  u64 ld;
+  double S, Q;
+  __device__ __forceinline__ void emit(u64 t, double d) {
+    if (MODE == kStoreStreamMajor) p[t] = d;
+    else if (MODE == kStoreInterleaved) __stcs(p + t * ld, d);
+    else { S = S + d; Q = __fma_rn(d, d, Q); }
+  }
+};
+
+template <int J, int MODE>
+struct EmitBlock {
+  // all 12 draws of block v go to output indices t0 .. t0 + 11
+  static __device__ __forceinline__ void all(Sink<MODE>& s, const u32 (&v)[18], u64 t0) {
+    if (MODE == kStoreStreamMajor) {
+      if (J % 2 == 0) {  // two draws per 128-bit store (p + t0 is 16-byte aligned: n_per % 12 == 0)
+        double2 d2 = make_double2(draw_double<J>(v), draw_double<J + 1>(v));
+        __stcs(reinterpret_cast<double2*>(s.p + t0 + J), d2);
+      }
+    } else {
+      s.emit(t0 + J, draw_double<J>(v));
+    }
+    EmitBlock<J + 1, MODE>::all(s, v, t0);
+  }
+  // draw J of the block at absolute draw position q0 + J is output index q0 + J - pos if in [0, n)
+  static __device__ __forceinline__ void masked(Sink<MODE>& s, const u32 (&v)[18], u64 q0, u32 pos, u64 n) {
+    const u64 t = q0 + J - pos;  // wraps when q0 + J < pos: then t >= n
+    const bool valid = t < n;
+    const double d = draw_double<J>(v);
+    if (MODE == kReduce) s.emit(t, valid ? d : 0.0);  // + 0.0 and fma(0, 0, Q) are exact no-ops
+    else if (valid) s.emit(t, d);
+    EmitBlock<J + 1, MODE>::masked(s, v, q0, pos, n);
+  }
+};
+template <int MODE>
+struct EmitBlock<12, MODE> {
+  static __device__ __forceinline__ void all(Sink<MODE>&, const u32 (&)[18], u64) {}
+  static __device__ __forceinline__ void masked(Sink<MODE>&, const u32 (&)[18], u64, u32, u64) {}
+};
+
+// ALIGNED: every cursor is 12 and n_per % 12 == 0: n_per / 12 advances, no masks.
+// General: draw t of a stream sits at absolute position q = pos + t counted from the start of
+// its current block; block s = q / 12 needs s advances (D8).  All threads run the same trip
+// count; a thread skips an advance only when it lies beyond its own last block.
+template <class Mult, int MODE, bool ALIGNED>
+__global__ void __launch_bounds__(kThreads) generate_kernel(const __grid_constant__ GenArgs a) {
+  const u64 il = (u64)blockIdx.x * kThreads + threadIdx.x;
+  if (il >= a.count) return;
+  const u64 i = a.first + il;
+  u32 x[18], v[18], pos, c;
+  load_state(a.st, a.n_total, i, x, pos);
+  const Mult mult(a.A);
+  Sink<MODE> sink;
+  sink.ld = a.ld;
+  sink.S = 0.0;
+  sink.Q = 0.0;
+  sink.p = MODE == kStoreStreamMajor ? a.out + il * a.n_per : (MODE == kStoreInterleaved ? a.out + il : nullptr);
+  const u64 n = a.n_per;
+  if (ALIGNED) {
+    const u64 nblk = n / 12;
+#pragma unroll 1
+    for (u64 b = 0; b < nblk; b++) {
+      mult.advance_block(x, v, c);
+      EmitBlock<0, MODE>::all(sink, v, b * 12);
+    }
+  } else if (n > 0) {
+    const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block (n >= 1)
+    // pos + n - 1 can exceed 64 bits only for n near 2^64, which no output buffer can hold
+    const u64 smax = (12 + (n - 1)) / 12;                                                // last block of any thread
+    if (pos < 12) {  // block 0 = the current block
+      to_ranlux_exact(x, v, c);
+      EmitBlock<0, MODE>::masked(sink, v, 0, pos, n);
+    }
+#pragma unroll 1
+    for (u64 s = 1; s <= smax; s++) {
+      if (s <= last) {
+        mult.advance_block(x, v, c);
+        EmitBlock<0, MODE>::masked(sink, v, s * 12, pos, n);
+      }
+    }
+    pos = (u32)((u64)pos + n - 12 * last);
+  }
+  store_state(a.st, a.n_total, i, x, pos);
+  if (MODE == kReduce) {
+    a.sum[il] = sink.S;
+    if (a.sumsq) a.sumsq[il] = sink.Q;
+  }
+}
+
+// Seeding and skip-ahead ("fast exponentiation by squaring"): x <- x * prod_b T[b]^(bit b of e)
+// with T[b] = base^(2^b) precomputed on the host (64 entries of 18 limbs).  A bit is processed by
+// the whole warp if any lane has it set; lanes without it keep their value.
+__device__ __forceinline__ void pow_table_mul(u32 (&x)[18], u64 e, const u32* __restrict__ table) {
+#pragma unroll 1
+  for (int b = 0; b < 64; b++) {
+    const bool bit = (e >> b) & 1;
+    if (!__any_sync(0xFFFFFFFFu, bit)) continue;
+    u32 t[18], r[18];
+#pragma unroll
+    for (int j = 0; j < 18; j++) t[j] = __ldg(table + b * 18 + j);
+    mulmod_generic(x, t, r);
+#pragma unroll
+    for (int j = 0; j < 18; j++) x[j] = bit ? r[j] : x[j];
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) seed_kernel(uint4* __restrict__ st, u64 n, u64 seed0,
+                                                        const u32* __restrict__ tableG) {
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  const bool live = i < n;
+  u32 x[18];
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = j == 0 ? 1u : 0u;
+  pow_table_mul(x, live ? seed0 + i : 0ull, tableG);  // D7: X = G^seed, start state 1
+  if (live) store_state(st, n, i, x, 12u);
+}
+
+__global__ void __launch_bounds__(kThreads) skip_kernel(uint4* __restrict__ st, u64 n, u64 n_uniform,
+                                                        const u64* __restrict__ n_each,
+                                                        const u32* __restrict__ tableA) {
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  const bool live = i < n;
+  u32 x[18], pos = 12;
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = 0;
+  if (live) load_state(st, n, i, x, pos);
+  const u64 nn = live ? (n_each ? n_each[i] : n_uniform) : 0ull;
+  u64 k = 0;
+  u32 newpos = pos;
+  if (nn > 0) {  // D8: k = floor((pos + nn - 1) / 12) without 64-bit overflow
+    const u64 t = nn - 1;
+    const u32 total = (u32)(t % 12) + pos;  // <= 23
+    k = t / 12 + total / 12;
+    newpos = total % 12 + 1;
+  }
+  pow_table_mul(x, k, tableA);
+  if (live) store_state(st, n, i, x, newpos);
+}
+
+// get_state: the paper's stored form: packed RANLUX numbers + carry, cursor, LCG state
+__global__ void __launch_bounds__(kThreads) export_kernel(const uint4* __restrict__ st, u64 n, u64* __restrict__ ranlux,
+                                                          u32* __restrict__ carry, u32* __restrict__ pos_out,
+                                                          u64* __restrict__ lcg) {
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  u32 x[18], v[18], pos, c;
+  load_state(st, n, i, x, pos);
+  to_ranlux_exact(x, v, c);
+#pragma unroll
+  for (int l = 0; l < 9; l++) {
+    if (ranlux) ranlux[i * 9 + l] = (u64)v[2 * l] | ((u64)v[2 * l + 1] << 32);
+    if (lcg) lcg[i * 9 + l] = (u64)x[2 * l] | ((u64)x[2 * l + 1] << 32);
+  }
+  if (carry) carry[i] = c;
+  if (pos_out) pos_out[i] = pos;
+}
+
+__global__ void __launch_bounds__(kThreads) import_kernel(uint4* __restrict__ st, u64 n, const u64* __restrict__ lcg,
+                                                          const u32* __restrict__ pos_in) {
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  u32 z[20], x[18];
+#pragma unroll
+  for (int l = 0; l < 9; l++) {
+    const u64 w = lcg[i * 9 + l];
+    z[2 * l] = (u32)w;
+    z[2 * l + 1] = (u32)(w >> 32);
+  }
+  z[18] = 0; z[19] = 0;
+  mod_m20(z, x);
+  u32 pos = pos_in ? pos_in[i] : 12u;
+  store_state(st, n, i, x, pos > 12u ? 12u : pos);
+}
+
+// ----------------------------------------------------------------------------- roofline probes
+// IMAD peak: 8 independent carry chains of IMAD.WIDE.U32.X per thread, nothing else in the loop.
+__global__ void __launch_bounds__(kThreads) imad_peak_kernel(u64* out, u32 iters, u32 seed) {
+  u64 acc[8];
+  u32 x = seed + threadIdx.x;
+#pragma unroll
+  for (int j = 0; j < 8; j++) acc[j] = (u64)seed * (j + 1);
+#pragma unroll 1
+  for (u32 it = 0; it < iters; it++) {
+#pragma unroll
+    for (int rep = 0; rep < 8; rep++) {
+      asm("{\n\t.reg .u64 t;\n\t"
+          "mul.wide.u32 t, %8, 0x9e3779b9; add.cc.u64  %0, %0, t;\n\t"
+          "mul.wide.u32 t, %8, 0x7f4a7c15; addc.cc.u64 %1, %1, t;\n\t"
+          "mul.wide.u32 t, %8, 0xbf58476d; addc.cc.u64 %2, %2, t;\n\t"
+          "mul.wide.u32 t, %8, 0x1ce4e5b9; addc.cc.u64 %3, %3, t;\n\t"
+          "mul.wide.u32 t, %8, 0x94d049bb; add.cc.u64  %4, %4, t;\n\t"
+          "mul.wide.u32 t, %8, 0x133111eb; addc.cc.u64 %5, %5, t;\n\t"
+          "mul.wide.u32 t, %8, 0xe220a839; addc.cc.u64 %6, %6, t;\n\t"
+          "mul.wide.u32 t, %8, 0x7b1dcdaf; addc.cc.u64 %7, %7, t;\n\t"
+          "}"
+          : "+l"(acc[0]), "+l"(acc[1]), "+l"(acc[2]), "+l"(acc[3]), "+l"(acc[4]), "+l"(acc[5]), "+l"(acc[6]), "+l"(acc[7])
+          : "r"(x));
+    }
+  }
+  u64 r = 0;
+#pragma unroll
+  for (int j = 0; j < 8; j++) r ^= acc[j];
+  if (r == 0x1234567u) out[0] = r;  // never true in practice; keeps the chains alive
+}
+constexpr int kImadPerIter = 64;
+
+__global__ void __launch_bounds__(256) hbm_write_kernel(uint4* __restrict__ out, u64 n16) {
+  const u64 stride = (u64)gridDim.x * blockDim.x;
+  const uint4 val = make_uint4(threadIdx.x, blockIdx.x, 0x3ff00000u, 0u);
+  for (u64 q = (u64)blockIdx.x * blockDim.x + threadIdx.x; q < n16; q += stride) __stcs(out + q, val);
+}
+
+// ----------------------------------------------------------------------------- host side
+struct Tables {
+  uint32_t p = 0;
+  Limbs18 A;
+  std::vector<uint32_t> tabA, tabG;  // [64][18]: A^(2^b), G^(2^b) with G = A^(2^96)
+};
+
+static void build_tables(uint32_t p, Tables& t, bool with_pow_tables) {
+  t.p = p;
+  host::Big A = host::multiplier_ap(p);
+  A.to_u32x18(t.A.v);
+  if (!with_pow_tables) return;
+  t.tabA.resize(64 * 18);
+  t.tabG.resize(64 * 18);
+  host::Big cur = A;
+  for (int b = 0; b < 64; b++) {
+    cur.to_u32x18(&t.tabA[b * 18]);
+    cur = host::mulmod(cur, cur);
+  }
+  cur = host::pow2k(A, 96);
+  for (int b = 0; b < 64; b++) {
+    cur.to_u32x18(&t.tabG[b * 18]);
+    cur = host::mulmod(cur, cur);
+  }
+}
+
+template <int P>
+static bool fixed_matches(const Limbs18& A) {
+  for (int j = 0; j < 18; j++)
+    if (FixedMultiplier<P>::kA[j] != A.v[j]) return false;
+  return true;
+}
+// which baked-in multiplier serves p (0 = none): the generated constants must equal the
+// host's own a^p, otherwise the header is stale and we refuse to use it
+static int fixed_level(uint32_t p, const Limbs18& A) {
+#define RLXPP_CASE(P) \
+  if (p == P) return fixed_matches<P>(A) ? P : -1;
+  RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
+#undef RLXPP_CASE
+  return 0;
+}
+
+}  // namespace rlx
+
+using namespace rlx;
+
+struct rlxpp {
+  uint64_t n = 0;
+  uint32_t p = 0;
+  int fixed = 0;
+  cudaStream_t stream = nullptr;
+  cudaStream_t copy_stream = nullptr;
+  uint4* st = nullptr;
+  uint32_t* tabA = nullptr;
+  uint32_t* tabG = nullptr;
+  Tables tables;
+  bool aligned = true;  // every cursor is known to be 12
+  uint32_t uniform_pos = 12;
+  bool pos_uniform = true;
+  // staging for the *_host variants
+  double* stage[2] = {nullptr, nullptr};
+  size_t stage_bytes = 0;
+  cudaEvent_t ev_kernel[2] = {nullptr, nullptr};
+  cudaEvent_t ev_copy[2] = {nullptr, nullptr};
+};
+
+static inline unsigned grid_for(uint64_t n) { return (unsigned)((n + kThreads - 1) / kThreads); }
+
+template <class Mult, int MODE>
+static int launch_generate_mode(const GenArgs& a, bool aligned, cudaStream_t s) {
+  if (aligned) generate_kernel<Mult, MODE, true><<<grid_for(a.count), kThreads, 0, s>>>(a);
+  else generate_kernel<Mult, MODE, false><<<grid_for(a.count), kThreads, 0, s>>>(a);
+  LAUNCH_CHECK();
+  return RLXPP_OK;
+}
+template <class Mult>
+static int launch_generate_mult(const GenArgs& a, int mode, bool aligned, cudaStream_t s) {
+  switch (mode) {
+    case kStoreStreamMajor: return launch_generate_mode<Mult, kStoreStreamMajor>(a, aligned, s);
+    case kStoreInterleaved: return launch_generate_mode<Mult, kStoreInterleaved>(a, aligned, s);
+    default: return launch_generate_mode<Mult, kReduce>(a, aligned, s);
+  }
+}
+static int launch_generate(int fixed, const GenArgs& a, int mode, bool aligned, cudaStream_t s) {
+#define RLXPP_CASE(P) \
+  if (fixed == P) return launch_generate_mult<Fixed<P>>(a, mode, aligned, s);
+  RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
+#undef RLXPP_CASE
+  return launch_generate_mult<Generic>(a, mode, aligned, s);
+}
+
+template <class Mult>
+static int launch_advance_mult(uint64_t* states, uint64_t n, uint32_t reps, int layout, const Limbs18& A,
+                               cudaStream_t s) {
+  if (layout == RLXPP_AOS) advance_states_kernel<Mult, RLXPP_AOS><<<grid_for(n), kThreads, 0, s>>>(states, n, reps, A);
+  else advance_states_kernel<Mult, RLXPP_SOA><<<grid_for(n), kThreads, 0, s>>>(states, n, reps, A);
+  LAUNCH_CHECK();
+  return RLXPP_OK;
+}
+
+static int check_device() {
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  return RLXPP_OK;
+}
+
+extern "C" {
+
+const char* rlxpp_last_error(void) { return g_last_error.c_str(); }
+const char* rlxpp_version(void) { return "rlxpp 0.1 (sm_100a)"; }
+uint64_t rlxpp_launch_count(void) { return g_launches.load(); }
+uint64_t rlxpp_n_streams(const rlxpp_t* h) { return h ? h->n : 0; }
+
+int rlxpp_has_fixed_multiplier(uint32_t p) {
+#define RLXPP_CASE(P) \
+  if (p == P) return 1;
+  RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
+#undef RLXPP_CASE
+  return 0;
+}
+
+int rlxpp_multiplier(uint32_t p, uint64_t* out_host) {
+  if (!out_host || p == 0) return fail(RLXPP_EINVAL, "rlxpp_multiplier: null output or p == 0");
+  host::multiplier_ap(p).to_u64x9(out_host);
+  return RLXPP_OK;
+}
+int rlxpp_seed_state(uint64_t seed, uint32_t p, uint64_t* out_host) {
+  if (!out_host || p == 0) return fail(RLXPP_EINVAL, "rlxpp_seed_state: null output or p == 0");
+  host::Big G = host::pow2k(host::multiplier_ap(p), 96);
+  host::powmod(G, seed).to_u64x9(out_host);
+  return RLXPP_OK;
+}
+
+int rlxpp_create(rlxpp_t** hout, uint64_t n_streams, uint64_t seed, uint32_t p, void* cuda_stream) {
+  if (!hout) return fail(RLXPP_EINVAL, "rlxpp_create: null handle pointer");
+  *hout = nullptr;
+  if (n_streams == 0) return fail(RLXPP_EINVAL, "rlxpp_create: n_streams == 0");
+  if (p == 0) return fail(RLXPP_EINVAL, "rlxpp_create: p == 0");
+  if (n_streams > (1ull << 31) * kThreads) return fail(RLXPP_EINVAL, "rlxpp_create: too many streams");
+  int rc = check_device();
+  if (rc) return rc;
+  rlxpp* h = new (std::nothrow) rlxpp();
+  if (!h) return fail(RLXPP_ENOMEM, "rlxpp_create: host allocation failed");
+  h->n = n_streams;
+  h->p = p;
+  h->stream = (cudaStream_t)cuda_stream;
+  build_tables(p, h->tables, true);
+  h->fixed = fixed_level(p, h->tables.A);
+  if (h->fixed < 0) {
+    delete h;
+    return fail(RLXPP_EINVAL, "rlxpp_create: rows_generated.cuh is stale for p = %u (rebuild)", p);
+  }
+  cudaError_t e = cudaMalloc(&h->st, sizeof(uint4) * 5 * n_streams);
+  if (e == cudaSuccess) e = cudaMalloc(&h->tabA, 64 * 18 * sizeof(uint32_t));
+  if (e == cudaSuccess) e = cudaMalloc(&h->tabG, 64 * 18 * sizeof(uint32_t));
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(h->tabA, h->tables.tabA.data(), 64 * 18 * sizeof(uint32_t), cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(h->tabG, h->tables.tabG.data(), 64 * 18 * sizeof(uint32_t), cudaMemcpyHostToDevice, h->stream);
+  if (e != cudaSuccess) {
+    int code = e == cudaErrorMemoryAllocation ? RLXPP_ENOMEM : RLXPP_ECUDA;
+    fail(code, "rlxpp_create: %s", cudaGetErrorString(e));
+    rlxpp_destroy(h);
+    return code;
+  }
+  seed_kernel<<<grid_for(n_streams), kThreads, 0, h->stream>>>(h->st, n_streams, seed, h->tabG);
+  g_launches++;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    fail(RLXPP_ECUDA, "rlxpp_create: seed kernel: %s", cudaGetErrorString(e));
+    rlxpp_destroy(h);
+    return RLXPP_ECUDA;
+  }
+  *hout = h;
+  return RLXPP_OK;
+}
+
+int rlxpp_destroy(rlxpp_t* h) {
+  if (!h) return RLXPP_OK;
+  if (h->stream || h->st) cudaStreamSynchronize(h->stream);
+  cudaFree(h->st);
+  cudaFree(h->tabA);
+  cudaFree(h->tabG);
+  for (int b = 0; b < 2; b++) {
+    cudaFree(h->stage[b]);
+    if (h->ev_kernel[b]) cudaEventDestroy(h->ev_kernel[b]);
+    if (h->ev_copy[b]) cudaEventDestroy(h->ev_copy[b]);
+  }
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  delete h;
+  return RLXPP_OK;
+}
+
+int rlxpp_skip(rlxpp_t* h, uint64_t n) {
+  if (!h) return fail(RLXPP_EINVAL, "rlxpp_skip: null handle");
+  if (n == 0) return RLXPP_OK;
+  skip_kernel<<<grid_for(h->n), kThreads, 0, h->stream>>>(h->st, h->n, n, nullptr, h->tabA);
+  LAUNCH_CHECK();
+  if (h->pos_uniform) {
+    const uint64_t t = n - 1;
+    const uint32_t total = (uint32_t)(t % 12) + h->uniform_pos;
+    h->uniform_pos = total % 12 + 1;
+  }
+  h->aligned = h->pos_uniform && h->uniform_pos == 12;
+  return RLXPP_OK;
+}
+
+int rlxpp_skip_each(rlxpp_t* h, const uint64_t* n_dev) {
+  if (!h || !n_dev) return fail(RLXPP_EINVAL, "rlxpp_skip_each: null argument");
+  skip_kernel<<<grid_for(h->n), kThreads, 0, h->stream>>>(h->st, h->n, 0, n_dev, h->tabA);
+  LAUNCH_CHECK();
+  h->pos_uniform = false;
+  h->aligned = false;
+  return RLXPP_OK;
+}
+
+int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, uint32_t reps, int layout,
+                         void* cuda_stream) {
+  if (p == 0) return fail(RLXPP_EINVAL, "rlxpp_advance_states: p == 0");
+  if (layout != RLXPP_AOS && layout != RLXPP_SOA) return fail(RLXPP_EINVAL, "rlxpp_advance_states: unknown layout %d", layout);
+  if (n_states == 0) return RLXPP_OK;
+  if (!states_dev) return fail(RLXPP_EINVAL, "rlxpp_advance_states: null states");
+  if ((uintptr_t)states_dev % 16) return fail(RLXPP_EINVAL, "rlxpp_advance_states: states must be 16-byte aligned");
+  int rc = check_device();
+  if (rc) return rc;
+  Tables t;
+  build_tables(p, t, false);
+  const int fixed = fixed_level(p, t.A);
+  if (fixed < 0) return fail(RLXPP_EINVAL, "rlxpp_advance_states: rows_generated.cuh is stale for p = %u", p);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+#define RLXPP_CASE(P) \
+  if (fixed == P) return launch_advance_mult<Fixed<P>>(states_dev, n_states, reps, layout, t.A, s);
+  RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
+#undef RLXPP_CASE
+  return launch_advance_mult<Generic>(states_dev, n_states, reps, layout, t.A, s);
+}
+
+static void after_generate(rlxpp_t* h, uint64_t n) {
+  if (h->pos_uniform && n > 0) {
+    const uint64_t t = n - 1;
+    const uint32_t total = (uint32_t)(t % 12) + h->uniform_pos;
+    h->uniform_pos = total % 12 + 1;
+  }
+  h->aligned = h->pos_uniform && h->uniform_pos == 12;
+}
+
+int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout) {
+  if (!h) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: null handle");
+  if (layout != RLXPP_STREAM_MAJOR && layout != RLXPP_INTERLEAVED)
+    return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: unknown layout %d", layout);
+  if (n_per_stream == 0) return RLXPP_OK;
+  if (!out_dev) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: null output");
+  if ((uintptr_t)out_dev % 16) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: output must be 16-byte aligned");
+  GenArgs a;
+  a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = out_dev; a.ld = h->n;
+  a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A;
+  const bool aligned = h->aligned && n_per_stream % 12 == 0;
+  int rc = launch_generate(h->fixed, a, layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved, aligned,
+                           h->stream);
+  if (rc) return rc;
+  after_generate(h, n_per_stream);
+  return RLXPP_OK;
+}
+
+int rlxpp_generate_reduce(rlxpp_t* h, double* sum_dev, double* sumsq_dev, uint64_t n_per_stream) {
+  if (!h || !sum_dev) return fail(RLXPP_EINVAL, "rlxpp_generate_reduce: null argument");
+  GenArgs a;
+  a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = nullptr; a.ld = 0;
+  a.n_per = n_per_stream; a.sum = sum_dev; a.sumsq = sumsq_dev; a.A = h->tables.A;
+  const bool aligned = h->aligned && n_per_stream % 12 == 0;
+  int rc = launch_generate(h->fixed, a, kReduce, aligned, h->stream);
+  if (rc) return rc;
+  after_generate(h, n_per_stream);
+  return RLXPP_OK;
+}
+
+static int ensure_staging(rlxpp_t* h, size_t bytes_each) {
+  if (!h->copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  for (int b = 0; b < 2; b++) {
+    if (!h->ev_kernel[b]) CUDA_TRY(cudaEventCreateWithFlags(&h->ev_kernel[b], cudaEventDisableTiming));
+    if (!h->ev_copy[b]) CUDA_TRY(cudaEventCreateWithFlags(&h->ev_copy[b], cudaEventDisableTiming));
+  }
+  if (h->stage_bytes < bytes_each) {
+    for (int b = 0; b < 2; b++) {
+      cudaFree(h->stage[b]);
+      h->stage[b] = nullptr;
+    }
+    h->stage_bytes = 0;
+    for (int b = 0; b < 2; b++) CUDA_TRY(cudaMalloc(&h->stage[b], bytes_each));
+    h->stage_bytes = bytes_each;
+  }
+  return RLXPP_OK;
+}
+
+int rlxpp_generate_doubles_host(rlxpp_t* h, double* out_host, uint64_t n_per_stream, int layout) {
+  if (!h) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles_host: null handle");
+  if (layout != RLXPP_STREAM_MAJOR && layout != RLXPP_INTERLEAVED)
+    return fail(RLXPP_EINVAL, "rlxpp_generate_doubles_host: unknown layout %d", layout);
+  if (n_per_stream == 0) return RLXPP_OK;
+  if (!out_host) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles_host: null output");
+  // chunks of streams, at most 512 MiB of doubles each, double-buffered: the kernel of chunk
+  // c+1 overlaps the device->host copy of chunk c
+  const uint64_t max_doubles = (512ull << 20) / 8;
+  uint64_t chunk = max_doubles / n_per_stream;
+  chunk = chunk / 1024 * 1024;
+  if (chunk == 0) chunk = kThreads;
+  if (chunk > h->n) chunk = h->n;
+  int rc = ensure_staging(h, chunk * n_per_stream * sizeof(double));
+  if (rc) return rc;
+  const bool aligned = h->aligned && n_per_stream % 12 == 0;
+  const int mode = layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved;
+  int buf = 0;
+  uint64_t done = 0;
+  for (uint64_t first = 0; first < h->n; first += chunk, buf ^= 1, done++) {
+    const uint64_t count = h->n - first < chunk ? h->n - first : chunk;
+    if (done >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copy[buf], 0));  // buffer free again
+    GenArgs a;
+    a.st = h->st; a.n_total = h->n; a.first = first; a.count = count; a.out = h->stage[buf]; a.ld = count;
+    a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A;
+    rc = launch_generate(h->fixed, a, mode, aligned, h->stream);
+    if (rc) return rc;
+    CUDA_TRY(cudaEventRecord(h->ev_kernel[buf], h->stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_kernel[buf], 0));
+    if (layout == RLXPP_STREAM_MAJOR) {
+      CUDA_TRY(cudaMemcpyAsync(out_host + first * n_per_stream, h->stage[buf], count * n_per_stream * sizeof(double),
+                               cudaMemcpyDeviceToHost, h->copy_stream));
+    } else {
+      CUDA_TRY(cudaMemcpy2DAsync(out_host + first, h->n * sizeof(double), h->stage[buf], count * sizeof(double),
+                                 count * sizeof(double), n_per_stream, cudaMemcpyDeviceToHost, h->copy_stream));
+    }
+    CUDA_TRY(cudaEventRecord(h->ev_copy[buf], h->copy_stream));
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  after_generate(h, n_per_stream);
+  return RLXPP_OK;
+}
+
+int rlxpp_generate_reduce_host(rlxpp_t* h, double* sum_host, double* sumsq_host, uint64_t n_per_stream) {
+  if (!h || !sum_host) return fail(RLXPP_EINVAL, "rlxpp_generate_reduce_host: null argument");
+  int rc = ensure_staging(h, 2 * h->n * sizeof(double));
+  if (rc) return rc;
+  double* s = h->stage[0];
+  double* q = h->stage[0] + h->n;
+  rc = rlxpp_generate_reduce(h, s, q, n_per_stream);
+  if (rc) return rc;
+  CUDA_TRY(cudaMemcpyAsync(sum_host, s, h->n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  if (sumsq_host) CUDA_TRY(cudaMemcpyAsync(sumsq_host, q, h->n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return RLXPP_OK;
+}
+
+int rlxpp_get_state(rlxpp_t* h, uint64_t* ranlux_dev, uint32_t* carry_dev, uint32_t* pos_dev, uint64_t* lcg_dev) {
+  if (!h) return fail(RLXPP_EINVAL, "rlxpp_get_state: null handle");
+  export_kernel<<<grid_for(h->n), kThreads, 0, h->stream>>>(h->st, h->n, ranlux_dev, carry_dev, pos_dev, lcg_dev);
+  LAUNCH_CHECK();
+  return RLXPP_OK;
+}
+
+int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev) {
+  if (!h || !lcg_dev) return fail(RLXPP_EINVAL, "rlxpp_set_state: null argument");
+  import_kernel<<<grid_for(h->n), kThreads, 0, h->stream>>>(h->st, h->n, lcg_dev, pos_dev);
+  LAUNCH_CHECK();
+  h->pos_uniform = pos_dev == nullptr;
+  h->uniform_pos = 12;
+  h->aligned = h->pos_uniform;
+  return RLXPP_OK;
+}
+
+int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream) {
+  if (!imad_per_s || iters <= 0) return fail(RLXPP_EINVAL, "rlxpp_measure_imad_peak: bad argument");
+  int rc = check_device();
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  u64* out = nullptr;
+  CUDA_TRY(cudaMalloc(&out, 64));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  const unsigned blocks = (unsigned)sms * 8;  // 8 x 128 threads per SM = 8 warps per scheduler
+  const u32 loop = 4096;
+  double best = 0.0;
+  for (int it = 0; it < iters + 2; it++) {
+    CUDA_TRY(cudaEventRecord(e0, s));
+    imad_peak_kernel<<<blocks, kThreads, 0, s>>>(out, loop, 12345u + it);
+    g_launches++;
+    CUDA_TRY(cudaEventRecord(e1, s));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    const double rate = (double)blocks * kThreads * loop * kImadPerIter / (ms * 1e-3);
+    if (it >= 2 && rate > best) best = rate;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  *imad_per_s = best;
+  return RLXPP_OK;
+}
+
+int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s, void* cuda_stream) {
+  if (!bytes_per_s || iters <= 0 || bytes < 16) return fail(RLXPP_EINVAL, "rlxpp_measure_hbm_write_peak: bad argument");
+  int rc = check_device();
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  uint4* buf = nullptr;
+  CUDA_TRY(cudaMalloc(&buf, bytes));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  double best = 0.0;
+  for (int it = 0; it < iters + 2; it++) {
+    CUDA_TRY(cudaEventRecord(e0, s));
+    hbm_write_kernel<<<sms * 8, 256, 0, s>>>(buf, bytes / 16);
+    g_launches++;
+    CUDA_TRY(cudaEventRecord(e1, s));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    const double rate = (double)(bytes / 16 * 16) / (ms * 1e-3);
+    if (it >= 2 && rate > best) best = rate;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(buf);
+  *bytes_per_s = best;
+  return RLXPP_OK;
+}
+
+}  // extern "C"
