@@ -1,0 +1,384 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element, tolerance 0 -- every step of RANLUX++ is exact integer arithmetic or exactly
+representable fp64, and the fused sums are evaluated in the same order
+with the same single-rounding fma on both sides (reading c-14).
+
+Small cases span several 128-thread blocks and a ragged tail and are compared in full; the
+BASELINE.json full sizes run in bench.py's launch configuration and are compared on sampled
+streams (the oracle computes any stream on its own) plus size-independent properties.
+"""
+import numpy as np
+import pytest
+
+from paper_2106_02504_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+M = (1 << 576) - (1 << 240) + 1
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as _torch
+    if not _torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device (there is no CPU fallback)")
+    return _torch
+
+
+@pytest.fixture(scope="module")
+def rlx(torch):
+    import paper_2106_02504_b200 as _rlx
+    _rlx.load()
+    return _rlx
+
+
+@pytest.fixture(scope="module")
+def nthreads(oracle):
+    return max(1, oracle.hardware_threads())
+
+
+def bits(a):
+    return np.ascontiguousarray(a).view(np.uint64)
+
+
+def assert_bits_equal(got, want, what):
+    g, w = bits(got), bits(want)
+    assert g.shape == w.shape, (what, g.shape, w.shape)
+    bad = np.nonzero(g != w)
+    assert bad[0].size == 0, f"{what}: {bad[0].size} mismatches, first at {[int(b[0]) for b in bad]}: " \
+                             f"got {g[tuple(b[0] for b in bad)]:#x} want {w[tuple(b[0] for b in bad)]:#x}"
+
+
+def gpu_state(rlx, torch, h):
+    n = h.n_streams
+    V = torch.empty((n, 9), dtype=torch.int64, device="cuda")
+    X = torch.empty((n, 9), dtype=torch.int64, device="cuda")
+    c = torch.empty(n, dtype=torch.int32, device="cuda")
+    pos = torch.empty(n, dtype=torch.int32, device="cuda")
+    rlx.rlxpp_get_state(h, V, c, pos, X)
+    torch.cuda.synchronize()
+    return (V.cpu().numpy().view(np.uint64), c.cpu().numpy().view(np.uint32), pos.cpu().numpy().view(np.uint32),
+            X.cpu().numpy().view(np.uint64))
+
+
+def check_state(rlx, torch, h, ref, what):
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    assert_bits_equal(X, ref["X"], what + " LCG state")
+    assert_bits_equal(V, ref["V"], what + " RANLUX numbers")
+    assert np.array_equal(c, ref["c"]), what + " carry"
+    assert np.array_equal(pos, ref["pos"]), what + " cursor"
+
+
+# ------------------------------------------------------------------------------------- host helpers
+def test_host_multiplier_and_seed_state_match_oracle(rlx, oracle):
+    for p in (1, 24, 389, 1024, 2048, 777):
+        assert inputs.limbs_to_int(rlx.rlxpp_multiplier(p)) == oracle.multiplier(p)
+    for seed, p in ((0, 2048), (1, 2048), (2**64 - 1, 2048), (12345, 24), (7, 389)):
+        assert inputs.limbs_to_int(rlx.rlxpp_seed_state(seed, p)) == oracle.seed_state(seed, p)
+
+
+# ------------------------------------------------------------------------------------- config 1
+def test_cfg1_smallest_instance_full_compare(rlx, torch, oracle, nthreads):
+    """BASELINE.json configs[0]: 1,024 streams, seeds 1..1024, p = 2048, 32 advances = 384 doubles per
+    stream, stream-major, all 393,216 doubles and the final states bit-exact."""
+    n, per = 1024, 384
+    h = rlx.rlxpp_create(n, 1, 2048)
+    out = torch.empty((n, per), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_STREAM_MAJOR)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n), 2048, per, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(out.cpu().numpy(), ref["doubles"], "cfg1 doubles")
+    check_state(rlx, torch, h, ref, "cfg1")
+    got = out.cpu().numpy()
+    assert got.min() >= 0.0 and got.max() < 1.0
+    assert np.array_equal(got * 2.0**48, np.floor(got * 2.0**48))  # the 2^-48 lattice
+    rlx.rlxpp_destroy(h)
+
+
+# ------------------------------------------------------------------------------------- config 2
+@pytest.mark.parametrize("layout", ["aos", "soa"])
+@pytest.mark.parametrize("p", [2048, 24, 100])
+def test_cfg2_advance_states_small(rlx, torch, oracle, nthreads, layout, p):
+    """Raw LCG advance: random states in [0, m), the 64 edge states (0, 1, m-1, m-2^240, [m, 2^576),
+    top limb all ones), 16 repetitions in place; n = 5,000 + 64 is not a multiple of the block size.
+    p = 100 takes the generic-multiplier kernel."""
+    states = inputs.cfg2_states(5000)
+    n = states.shape[0]
+    want = oracle.advance_states(states, p, 16, nthreads)
+    if layout == "aos":
+        dev = torch.from_numpy(states.view(np.int64)).cuda()
+        rlx.rlxpp_advance_states(dev, n, p, 16, rlx.RLXPP_AOS)
+        got = dev.cpu().numpy().view(np.uint64)
+    else:
+        dev = torch.from_numpy(np.ascontiguousarray(states.T).view(np.int64)).cuda()
+        rlx.rlxpp_advance_states(dev, n, p, 16, rlx.RLXPP_SOA)
+        got = np.ascontiguousarray(dev.cpu().numpy().view(np.uint64).T)
+    assert_bits_equal(got, want, f"cfg2 {layout} p={p}")
+    assert all(inputs.limbs_to_int(r) < M for r in got[-64:])
+
+
+def test_cfg2_reps_zero_canonicalises_and_empty_is_noop(rlx, torch, oracle):
+    states = inputs.cfg2_edge_states()
+    dev = torch.from_numpy(states.view(np.int64)).cuda()
+    rlx.rlxpp_advance_states(dev, 64, 2048, 0, rlx.RLXPP_AOS)
+    got = dev.cpu().numpy().view(np.uint64)
+    for g, s in zip(got, states):
+        assert inputs.limbs_to_int(g) == inputs.limbs_to_int(s) % M
+    rlx.rlxpp_advance_states(dev, 0, 2048, 16, rlx.RLXPP_AOS)  # n == 0
+    assert np.array_equal(dev.cpu().numpy().view(np.uint64), got)
+    one = torch.from_numpy(states[:1].copy().view(np.int64)).cuda()  # a single state (9 words: odd tail)
+    rlx.rlxpp_advance_states(one, 1, 2048, 3, rlx.RLXPP_AOS)
+    assert_bits_equal(one.cpu().numpy(), oracle.advance_states(states[:1], 2048, 3), "single state")
+
+
+def test_cfg2_full_size(rlx, torch, oracle, nthreads):
+    """BASELINE.json configs[1] at full size: 2^20 + 64 states x 16 advances, every state compared."""
+    states = inputs.cfg2_states(1 << 20)
+    n = states.shape[0]
+    dev = torch.from_numpy(states.view(np.int64)).cuda()
+    rlx.rlxpp_advance_states(dev, n, 2048, 16, rlx.RLXPP_AOS)
+    got = dev.cpu().numpy().view(np.uint64)
+    want = oracle.advance_states(states, 2048, 16, nthreads)
+    assert_bits_equal(got, want, "cfg2 full")
+
+
+# ------------------------------------------------------------------------------------- config 3
+def test_cfg3_interleaved_small(rlx, torch, oracle, nthreads):
+    n, per = 1000, 1536  # 7 full blocks + a ragged one; 128 advances per stream
+    h = rlx.rlxpp_create(n, 1, 2048)
+    out = torch.empty((per, n), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n), 2048, per, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(out.cpu().numpy().T, ref["doubles"], "cfg3 small")
+    check_state(rlx, torch, h, ref, "cfg3 small")
+
+
+def test_cfg3_full_size_sampled(rlx, torch, oracle, nthreads):
+    """BASELINE.json configs[2] in bench.py's launch configuration: 2^20 streams x 1,536 doubles,
+    interleaved, 12.9 GB.  Sampled streams (first and last blocks, a stride through the rest) are
+    compared in full; the whole array is checked for range and lattice on the device."""
+    n, per = 1 << 20, 1536
+    h = rlx.rlxpp_create(n, 1, 2048)
+    out = torch.empty((per, n), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+    torch.cuda.synchronize()
+    idx = np.unique(np.concatenate([np.arange(0, 130), np.arange(n - 130, n), np.arange(0, n, 4099)]))
+    got = out[:, torch.from_numpy(idx).cuda()].cpu().numpy().T
+    ref = oracle.streams(inputs.seeds(n)[idx], 2048, per, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(got, ref["doubles"], "cfg3 full (sampled streams)")
+    for lo in range(0, per, 128):  # properties at any size, chunked to bound temporaries
+        blk = out[lo:lo + 128]
+        assert bool((blk >= 0).all()) and bool((blk < 1).all())
+        sc = blk * 2.0**48
+        assert bool((sc == sc.floor()).all())
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    assert_bits_equal(X[idx], ref["X"], "cfg3 full state")
+    assert np.all(pos == 12)
+    del out
+
+
+# ------------------------------------------------------------------------------------- config 4
+@pytest.mark.parametrize("p", [24, 389, 1024, 2048])
+def test_cfg4_luxury_sweep_small(rlx, torch, oracle, nthreads, p):
+    n, per = 700, 6144
+    h = rlx.rlxpp_create(n, 1, p)
+    out = torch.empty((per, n), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n), p, per, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(out.cpu().numpy().T, ref["doubles"], f"cfg4 p={p}")
+    check_state(rlx, torch, h, ref, f"cfg4 p={p}")
+
+
+def test_cfg4_p24_is_direct_subtract_with_borrow(rlx, torch, oracle):
+    """p = 24 skips nothing: the GPU stream must be the raw RANLUX (SWB) sequence started from the
+    seeded state (reading c-13), here produced by the oracle's direct SWB stepper."""
+    n, per = 64, 120
+    h = rlx.rlxpp_create(n, 1, 24)
+    out = torch.empty((n, per), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_STREAM_MAJOR)
+    got = (out.cpu().numpy() * 2.0**48).astype(np.uint64)
+    for i in (0, 1, 63):
+        V, c = oracle.to_ranlux(oracle.seed_state(1 + i, 24))
+        want = []
+        for _ in range(per // 12):
+            V, c = oracle.swb_steps(V, c, 24)
+            want += [(V >> (48 * j)) & (2**48 - 1) for j in range(12)]
+        assert [int(v) for v in got[i]] == want
+
+
+@pytest.mark.parametrize("p", [24, 389, 1024, 2048])
+def test_cfg4_full_size_sampled(rlx, torch, oracle, nthreads, p):
+    n, per = 1 << 18, 6144
+    h = rlx.rlxpp_create(n, 1, p)
+    out = torch.empty((per, n), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+    torch.cuda.synchronize()
+    idx = np.unique(np.concatenate([np.arange(0, 40), np.arange(n - 40, n), np.arange(0, n, 2731)]))
+    got = out[:, torch.from_numpy(idx).cuda()].cpu().numpy().T
+    ref = oracle.streams(inputs.seeds(n)[idx], p, per, want=("doubles",), nthreads=nthreads)
+    assert_bits_equal(got, ref["doubles"], f"cfg4 full p={p}")
+    del out
+
+
+# ------------------------------------------------------------------------------------- config 5
+def test_cfg5_skip_and_fused_reduce_small(rlx, torch, oracle, nthreads):
+    n, per = 3000, 49152 // 8
+    dist = inputs.cfg5_skip_distances(n)
+    h = rlx.rlxpp_create(n, 1, 2048)
+    rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    s = torch.empty(n, dtype=torch.float64, device="cuda")
+    q = torch.empty(n, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_reduce(h, s, q, per)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n), 2048, per, skips=dist, want=("sums", "state"), nthreads=nthreads)
+    assert_bits_equal(s.cpu().numpy(), ref["sum"], "cfg5 sum")
+    assert_bits_equal(q.cpu().numpy(), ref["sumsq"], "cfg5 sum of squares")
+    check_state(rlx, torch, h, ref, "cfg5 small")
+
+
+def test_cfg5_full_size_sampled(rlx, torch, oracle, nthreads):
+    """BASELINE.json configs[4]: 2^18 streams, random 64-bit skips, 49,152 doubles each reduced in
+    registers.  The oracle recomputes a sample of streams (each 4,096 advances)."""
+    n, per = 1 << 18, 49152
+    dist = inputs.cfg5_skip_distances(n)
+    h = rlx.rlxpp_create(n, 1, 2048)
+    rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    s = torch.empty(n, dtype=torch.float64, device="cuda")
+    q = torch.empty(n, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_reduce(h, s, q, per)
+    torch.cuda.synchronize()
+    idx = np.unique(np.concatenate([np.arange(0, 33), np.arange(n - 33, n), np.arange(0, n, 257)]))
+    ref = oracle.streams(inputs.seeds(n)[idx], 2048, per, skips=dist[idx], want=("sums", "state"), nthreads=nthreads)
+    assert_bits_equal(s.cpu().numpy()[idx], ref["sum"], "cfg5 full sum")
+    assert_bits_equal(q.cpu().numpy()[idx], ref["sumsq"], "cfg5 full sumsq")
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    assert_bits_equal(X[idx], ref["X"], "cfg5 full state")
+    assert np.array_equal(pos[idx], ref["pos"])
+    sn = s.cpu().numpy()
+    assert np.all(sn > 0.4 * per) and np.all(sn < 0.6 * per)  # every stream was reduced
+
+
+# ------------------------------------------------------------------------------------- cursor logic
+def test_unaligned_draw_counts_and_uniform_skip(rlx, torch, oracle, nthreads):
+    """Draw counts that are not multiples of 12, interleaved with uniform skips (D8): the
+    concatenation must equal the oracle's engine driven with the same operations."""
+    n = 300
+    h = rlx.rlxpp_create(n, 77, 2048)
+    ops = [("draw", 7), ("draw", 5), ("skip", 1), ("draw", 13), ("skip", 12), ("draw", 1), ("skip", 2**40 + 5),
+           ("draw", 30), ("draw", 0), ("skip", 0), ("draw", 12), ("draw", 24), ("skip", 2**64 - 1), ("draw", 3)]
+    chunks = []
+    for kind, k in ops:
+        if kind == "skip":
+            rlx.rlxpp_skip(h, k)
+        else:
+            out = torch.full((n, max(k, 1)), -1.0, dtype=torch.float64, device="cuda")
+            rlx.rlxpp_generate_doubles(h, out, k, rlx.RLXPP_STREAM_MAJOR)
+            if k:
+                chunks.append(out.cpu().numpy())
+            else:
+                assert bool((out == -1.0).all())
+    got = (np.concatenate(chunks, axis=1) * 2.0**48).astype(np.uint64)
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    for i in (0, 1, 127, 128, 299):
+        X0 = oracle.seed_state(77 + i, 2048)
+        Xe, pe, draws = oracle.engine_run(X0, 12, 2048, ops)
+        assert [int(v) for v in got[i]] == draws
+        assert inputs.limbs_to_int(X[i]) == Xe and int(pos[i]) == pe
+
+
+def test_unaligned_interleaved_and_reduce_after_per_stream_skips(rlx, torch, oracle, nthreads):
+    n, per = 515, 100
+    dist = inputs.splitmix64(99, n) % np.uint64(40)  # small distances: every cursor value occurs
+    h = rlx.rlxpp_create(n, 5, 389)
+    rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    out = torch.empty((per, n), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+    ref = oracle.streams(inputs.seeds(n, 5), 389, per, skips=dist, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(out.cpu().numpy().T, ref["doubles"], "unaligned interleaved")
+    check_state(rlx, torch, h, ref, "unaligned interleaved")
+    s = torch.empty(n, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_reduce(h, s, None, 31)  # sumsq omitted
+    ref2 = oracle.streams(inputs.seeds(n, 5), 389, per + 31, skips=dist, want=("doubles",), nthreads=nthreads)
+    want = np.zeros(n)
+    for t in range(per, per + 31):
+        want = want + ref2["doubles"][:, t]
+    assert_bits_equal(s.cpu().numpy(), want, "reduce after unaligned draws")
+
+
+def test_generic_multiplier_streams(rlx, torch, oracle, nthreads):
+    """A luxury level without baked-in rows (p = 100) runs the full multiply9x9 + mod_m kernels."""
+    assert not rlx.rlxpp_has_fixed_multiplier(100)
+    n, per = 260, 60
+    h = rlx.rlxpp_create(n, 2**64 - 3, 100)  # seeds wrap mod 2^64
+    out = torch.empty((n, per), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_STREAM_MAJOR)
+    ref = oracle.streams(inputs.seeds(n, 2**64 - 3), 100, per, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(out.cpu().numpy(), ref["doubles"], "generic p=100")
+    check_state(rlx, torch, h, ref, "generic p=100")
+
+
+# ------------------------------------------------------------------------------------- state I/O
+def test_set_state_edge_states_and_roundtrip(rlx, torch, oracle):
+    """Import crafted LCG states (incl. 0, m-1, values >= m and the to_ranlux boundary cases), export
+    them in the paper's stored form and draw one block from each."""
+    edge = [0, 1, 2, M - 1, M - 2, M, M + 5, 2**576 - 1, M - (1 << 240), 1 << 240, (1 << 336) - 1, 1 << 336,
+            (1 << 336) + 1, (1 << 575), ((1 << 240) - 1) << 336, (((1 << 240) - 1) << 336) + (1 << 336) - 1]
+    rng = np.random.default_rng(3)
+    for _ in range(200):  # Xl + Xh near 2^336 and D near 0 (reading D4 / c-4)
+        xh = int.from_bytes(rng.bytes(30), "little")
+        edge.append(((xh << 336) + ((1 << 336) - xh + int(rng.integers(-2, 3)))) % 2**576)
+        edge.append(((xh << 336) + (xh << 96) + int(rng.integers(0, 2**20))) % 2**576)
+    n = len(edge)
+    states = np.stack([inputs.int_to_limbs(x) for x in edge])
+    h = rlx.rlxpp_create(n, 1, 2048)
+    rlx.rlxpp_set_state(h, torch.from_numpy(states.view(np.int64)).cuda(), None)
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    for i, x in enumerate(edge):
+        xc = x % M
+        assert inputs.limbs_to_int(X[i]) == xc
+        Vo, co = oracle.to_ranlux(xc)
+        assert inputs.limbs_to_int(V[i]) == Vo and int(c[i]) == co, f"to_ranlux edge {i}"
+    out = torch.empty((n, 12), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, 12, rlx.RLXPP_STREAM_MAJOR)
+    got = (out.cpu().numpy() * 2.0**48).astype(np.uint64)
+    A = oracle.multiplier(2048)
+    for i, x in enumerate(edge):
+        Vo, _ = oracle.to_ranlux(oracle.mulmod(A, x % M))
+        assert [int(v) for v in got[i]] == [(Vo >> (48 * j)) & (2**48 - 1) for j in range(12)]
+
+
+# ------------------------------------------------------------------------------------- host variants
+def test_host_destination_variants(rlx, torch, oracle, nthreads):
+    n, per = 2100, 48
+    ref = oracle.streams(inputs.seeds(n), 2048, per, want=("doubles", "sums"), nthreads=nthreads)
+    for layout in (rlx.RLXPP_STREAM_MAJOR, rlx.RLXPP_INTERLEAVED):
+        h = rlx.rlxpp_create(n, 1, 2048)
+        shape = (n, per) if layout == rlx.RLXPP_STREAM_MAJOR else (per, n)
+        out = torch.empty(shape, dtype=torch.float64).pin_memory()
+        rlx.rlxpp_generate_doubles_host(h, out, per, layout)
+        got = out.numpy() if layout == rlx.RLXPP_STREAM_MAJOR else out.numpy().T
+        assert_bits_equal(got, ref["doubles"], f"host variant layout {layout}")
+    h = rlx.rlxpp_create(n, 1, 2048)
+    s = np.zeros(n)
+    q = np.zeros(n)
+    rlx.rlxpp_generate_reduce_host(h, s, q, per)
+    assert_bits_equal(s, ref["sum"], "host reduce sum")
+    assert_bits_equal(q, ref["sumsq"], "host reduce sumsq")
+
+
+def test_errors_are_reported_not_swallowed(rlx, torch):
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_create(0, 1, 2048)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_create(10, 1, 0)
+    h = rlx.rlxpp_create(10, 1, 2048)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_generate_doubles(h, None, 12, rlx.RLXPP_STREAM_MAJOR)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_generate_doubles(h, torch.empty(120, dtype=torch.float64, device="cuda"), 12, 7)
+    assert "layout" in rlx.rlxpp_last_error()
+    before = rlx.rlxpp_launch_count()
+    rlx.rlxpp_generate_doubles(h, torch.empty(120, dtype=torch.float64, device="cuda"), 12, rlx.RLXPP_STREAM_MAJOR)
+    assert rlx.rlxpp_launch_count() == before + 1
