@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- RANLUX++ p = 2048 doubles/s on B200 through the C ABI (include/rlxpp.h).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|cfg4|cfg5] [--impl reference]
+
+One step = one pass of the whole hot path (load state, multiply9x9 by a^2048, mod_m, to_ranlux,
+12 doubles per advance, store) over one batch: BASELINE.json configs[2] ("bulk generation to
+HBM": 2^20 streams x 1,536 doubles, stream-interleaved, 12.9 GB written per step per GPU), the
+configuration the metric "doubles/sec" is quoted on.  Output (12.9 GB) is far larger than the
+126 MB L2, so no flush is needed between steps.  For N > 1 every rank owns its own 2^20 streams
+(seeds offset by rank * 2^20): weak scaling, no data-path collective (streams are independent,
+PAPER.md line 172).
+
+Prints ONE JSON line (rank 0).  DESIGN.md "Measurement" explains every key.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "RANLUX++ p=2048 doubles/sec"
+UNIT = "doubles/s"
+IMAD_PER_ADVANCE = 324  # 18 x 18 products 32x32->64 (81 products 64x64->128)
+IMAD_PER_DOUBLE = 27    # 324 / 12 (one LCG operation per 12 numbers)
+SM_COUNT = 148
+IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles per SMSP, 4 SMSPs
+
+WORKLOADS = {
+    # name: (streams, doubles per stream, p, description)
+    "cfg3": (1 << 20, 1536, 2048, "BASELINE configs[2]: 2^20 streams x 1536 doubles, p=2048, interleaved, 12.9 GB/step"),
+    "cfg4": (1 << 18, 6144, 2048, "BASELINE configs[3] at p=2048: 2^18 streams x 6144 doubles, interleaved, 12.9 GB/step"),
+    "cfg5": (1 << 18, 49152, 2048, "BASELINE configs[4]: 2^18 streams, random 64-bit skips, 49152 doubles fused to sum/sumsq"),
+    "cfg2": ((1 << 20) + 64, 16, 2048, "BASELINE configs[1]: 2^20+64 raw states x 16 advances in place (AoS)"),
+}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return d.get("hbm_gbs", 6650.0), d.get("sm_max_mhz", 1965.0), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi sampling DURING the timed region (B200_PROFILING.md clocks line)."""
+
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        res = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return res
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 9:
+                continue
+            try:
+                sm.append(float(parts[1]))
+                mx.append(float(parts[2]))
+                pw.append(float(parts[3]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            s = sorted(sm)
+            res.update(sm_mhz=s[len(s) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw))
+        return res
+
+
+def oracle_sample_rate(n_per, p, target_cpu_seconds=15.0):
+    """Times the oracle as it stands on a bounded sample of the same workload."""
+    import numpy as np
+    import oracle
+    from paper_2106_02504_b200 import inputs
+    cores = max(1, oracle.hardware_threads())
+    probe = 16 * cores
+    t0 = time.perf_counter()
+    oracle.streams(inputs.seeds(probe), p, n_per, want=("doubles",), nthreads=cores)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    per_stream_cpu = dt * cores / probe  # includes seeding (one powmod per stream)
+    n = int(min(max(target_cpu_seconds / per_stream_cpu, probe), 1 << 20))
+    n = max(cores, n // cores * cores)
+    t0 = time.perf_counter()
+    out = oracle.streams(inputs.seeds(n), p, n_per, want=("doubles",), nthreads=cores)["doubles"]
+    dt = time.perf_counter() - t0
+    assert out.shape == (n, n_per) and float(np.max(out)) < 1.0
+    return n * n_per / dt, cores, n, dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (oracle/), unmodified, on the host cores; each step is a
+    bounded sample of the workload (same p, same doubles per stream, fewer streams)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_2106_02504_b200 import inputs
+    n_streams, n_per, p, desc = WORKLOADS[args.workload]
+    if args.workload == "cfg2":
+        n_per = 12 * 16
+    cores = max(1, oracle.hardware_threads())
+    # size a step for ~3 s of wall clock
+    probe = 8 * cores
+    t0 = time.perf_counter()
+    oracle.streams(inputs.seeds(probe), p, n_per, want=("doubles",), nthreads=cores)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    budget = min(3.0, 150.0 / max(1, args.steps + args.warmup))
+    n = int(max(cores, min(n_streams, probe * budget / dt)))
+    n = max(cores, n // cores * cores)
+    for _ in range(args.warmup):
+        oracle.streams(inputs.seeds(n), p, n_per, want=("doubles",), nthreads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.streams(inputs.seeds(n), p, n_per, want=("doubles",), nthreads=cores)
+    dt = time.perf_counter() - t0
+    value = n * n_per * args.steps / dt
+    sample = f"{n} of {n_streams} streams x {n_per} doubles per step (seeding included), {cores} threads"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u64 integer limbs (unsigned __int128 products) -> f64", "data": "synthetic",
+        "config": {"workload": args.workload, "description": desc, "sampled": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import paper_2106_02504_b200 as rlx
+    from paper_2106_02504_b200 import inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rlx.load()
+
+    n_streams, n_per, p, desc = WORKLOADS[args.workload]
+    first_seed = 1 + rank * n_streams  # rank g owns seeds 1 + g N .. (g + 1) N
+    stream = torch.cuda.current_stream()
+
+    # ---------------------------------------------------------------- set up the step
+    if args.workload in ("cfg3", "cfg4"):
+        h = rlx.rlxpp_create(n_streams, first_seed, p)
+        out = torch.empty((n_per, n_streams), dtype=torch.float64, device="cuda")
+        units = n_streams * n_per
+        alg_bytes = units * 8 + 2 * 80 * n_streams  # doubles written + state read and written back
+        kernel = "generate_kernel<Fixed<2048>, interleaved, aligned>"
+
+        def step():
+            rlx.rlxpp_generate_doubles(h, out, n_per, rlx.RLXPP_INTERLEAVED)
+    elif args.workload == "cfg5":
+        h = rlx.rlxpp_create(n_streams, first_seed, p)
+        sk = torch.from_numpy(inputs.cfg5_skip_distances(n_streams).view(np.int64)).cuda()
+        rlx.rlxpp_skip_each(h, sk)
+        S = torch.empty(n_streams, dtype=torch.float64, device="cuda")
+        Q = torch.empty(n_streams, dtype=torch.float64, device="cuda")
+        units = n_streams * n_per
+        alg_bytes = (2 * 80 + 16) * n_streams
+        kernel = "generate_kernel<Fixed<2048>, reduce, unaligned>"
+
+        def step():
+            rlx.rlxpp_generate_reduce(h, S, Q, n_per)
+    else:  # cfg2: raw advances; "doubles" = 12 per advance for the common unit
+        h = None
+        states = torch.from_numpy(inputs.cfg2_states(1 << 20).view(np.int64)).cuda()
+        reps = n_per
+        units = n_streams * reps * 12
+        alg_bytes = 144 * n_streams
+        kernel = "advance_states_kernel<Fixed<2048>, AoS>"
+
+        def step():
+            rlx.rlxpp_advance_states(states, n_streams, p, reps, rlx.RLXPP_AOS)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------------------------------------------------------- warm-up + timed region
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    launches0 = rlx.rlxpp_launch_count()
+    barrier()
+    ev[0].record(stream)
+    for k in range(args.steps):
+        step()
+        ev[k + 1].record(stream)
+    barrier()
+    launches = rlx.rlxpp_launch_count() - launches0
+    clocks = sampler.stop() if sampler else {}
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = units * world / (ms_per_step * 1e-3)
+
+    # ---------------------------------------------------------------- roofline of the dominant kernel
+    hbm_gbs, sm_max_mhz, peak_src = peaks()
+    kernel_ms = sum(per_launch_ms) / len(per_launch_ms)  # one launch per step: event pairs bracket single launches
+    imad_nominal = SM_COUNT * IMAD_LANES_PER_CLK_SM * sm_max_mhz * 1e6  # IMAD/s at max clock
+    imad_achieved = units * IMAD_PER_DOUBLE / (kernel_ms * 1e-3)
+    hbm_achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
+    roof_alu = imad_nominal / IMAD_PER_DOUBLE
+    roof_hbm = hbm_gbs * 1e9 / 8 if args.workload in ("cfg3", "cfg4") else float("inf")
+    roofline = {
+        "bound": "alu", "kernel": kernel, "achieved": imad_achieved / 1e9, "peak": imad_nominal / 1e9, "unit": "GIMAD/s",
+        "frac": imad_achieved / imad_nominal, "traffic": None,
+        "peak_source": f"{SM_COUNT} SMs x {IMAD_LANES_PER_CLK_SM} IMAD lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md); "
+                       f"HBM {peak_src}",
+        "kernel_ms": kernel_ms,
+        "hbm": {"achieved": hbm_achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_achieved / hbm_gbs,
+                "algorithmic_bytes_per_launch": alg_bytes},
+        "doubles_roofline": {"alu": roof_alu, "hbm": (None if roof_hbm == float("inf") else roof_hbm),
+                             "min": min(roof_alu, roof_hbm), "frac": (units / (kernel_ms * 1e-3)) / min(roof_alu, roof_hbm)},
+    }
+    if clocks.get("sm_mhz"):
+        at_clock = SM_COUNT * IMAD_LANES_PER_CLK_SM * clocks["sm_mhz"] * 1e6
+        roofline["frac_at_observed_clock"] = imad_achieved / at_clock
+    if rank == 0:
+        try:
+            roofline["imad_microbench_peak"] = rlx.rlxpp_measure_imad_peak(3) / 1e9
+            roofline["frac_of_imad_microbench"] = imad_achieved / 1e9 / roofline["imad_microbench_peak"]
+            roofline["hbm_write_microbench_peak"] = rlx.rlxpp_measure_hbm_write_peak(8 << 30, 3) / 1e9
+        except rlx.RlxppError as e:  # the probes are context, the headline does not depend on them
+            roofline["probe_error"] = str(e)
+    traffic_file = os.path.join(ROOT, "profiles", "traffic_r01.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            roofline["traffic"] = json.load(f).get(args.workload)
+
+    # ---------------------------------------------------------------- end to end (host buffers)
+    e2e = None
+    if not args.no_e2e and args.workload in ("cfg3", "cfg4", "cfg5"):
+        if h is not None:
+            rlx.rlxpp_destroy(h)
+            h = None
+        if args.workload != "cfg5":
+            del out
+            torch.cuda.empty_cache()
+            host = torch.empty((n_per, n_streams), dtype=torch.float64, pin_memory=True)
+            d2h = n_streams * n_per * 8
+            h2d = 2 * 64 * 18 * 4  # the two power tables of the seeding / skip kernels
+
+            def e2e_step():
+                hh = rlx.rlxpp_create(n_streams, first_seed, p)
+                rlx.rlxpp_generate_doubles_host(hh, host, n_per, rlx.RLXPP_INTERLEAVED)
+                rlx.rlxpp_destroy(hh)
+        else:
+            hostS = torch.empty(n_streams, dtype=torch.float64, pin_memory=True)
+            hostQ = torch.empty(n_streams, dtype=torch.float64, pin_memory=True)
+            hsk = torch.from_numpy(inputs.cfg5_skip_distances(n_streams).view(np.int64)).pin_memory()
+            d2h = 16 * n_streams
+            h2d = 8 * n_streams + 2 * 64 * 18 * 4
+
+            def e2e_step():
+                hh = rlx.rlxpp_create(n_streams, first_seed, p)
+                dsk = hsk.cuda(non_blocking=True)
+                rlx.rlxpp_skip_each(hh, dsk)
+                rlx.rlxpp_generate_reduce_host(hh, hostS, hostQ, n_per)
+                rlx.rlxpp_destroy(hh)
+        e2e_step()  # warm-up (also pins / allocates the staging buffers' pages)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": units * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": args.e2e_steps,
+               "what": "rlxpp_create (seed kernel) + rlxpp_generate_*_host into pinned host memory + rlxpp_destroy, wall clock"}
+
+    # ---------------------------------------------------------------- oracle on the host cores
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        per = n_per if args.workload != "cfg2" else 12 * 16
+        v, cores, ns, dt = oracle_sample_rate(per, p)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{ns} of {n_streams} streams x {per} doubles (seeding included), {dt:.2f} s wall on {cores} threads"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64", "data": "synthetic",
+            "config": {"workload": args.workload, "description": desc, "n_streams_per_gpu": n_streams,
+                       "doubles_per_stream": n_per, "p": p, "l2": "output per step (12.9 GB) exceeds L2; no flush needed"
+                       if args.workload in ("cfg3", "cfg4") else "compute-bound; working set is registers",
+                       "parallelism": f"streams sharded over {world} GPU(s), no collective"},
+            "lcg_advances_per_s": value / 12.0,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
