@@ -48,6 +48,15 @@ extern "C" {
 #define RLXPP_AOS 0 /* states[i * 9 + limb] */
 #define RLXPP_SOA 1 /* states[limb * n_states + i] */
 
+/* engines of the LCG advance (multiply9x9 + mod_m, P:29 / P:33) used by rlxpp_advance_states and
+ * rlxpp_generate_*; both give bit-identical results:
+ *   UMMA (default): u8 x u8 -> s32 tensor-core GEMM against the byte matrix of A 2^(8k) mod m
+ *                   (tcgen05.mma kind::i8, 128 streams per CTA), any luxury level;
+ *   IMAD:           324 IMAD.WIDE.U32.X per advance with the multiplier as immediates
+ *                   (p in {24, 389, 1024, 2048}), generic 36-limb product otherwise. */
+#define RLXPP_ENGINE_UMMA 0
+#define RLXPP_ENGINE_IMAD 1
+
 typedef struct rlxpp rlxpp_t;
 
 /* Creates n_streams streams for luxury level p; stream i is seeded with seed + i
@@ -109,6 +118,15 @@ int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev
  * and the seed state (A^(2^96))^seed mod m.  out: 9 uint64_t on the host. */
 int rlxpp_multiplier(uint32_t p, uint64_t* out_host);
 int rlxpp_seed_state(uint64_t seed, uint32_t p, uint64_t* out_host);
+/* The byte matrix of the UMMA engine for luxury level p, as the host builds it:
+ * out_host[n * 72 + k] = byte n of (A 2^(8k) mod m), n, k in [0, 72) (5,184 bytes), so that for
+ * every x < 2^576 with bytes xb_k:  sum_n (sum_k xb_k out[n][k]) 2^(8n) == A x (mod m). */
+int rlxpp_umma_matrix(uint32_t p, uint8_t* out_host);
+
+/* Selects the engine for all later calls of this process (default RLXPP_ENGINE_UMMA).
+ * Errors: EINVAL for an unknown engine. */
+int rlxpp_set_engine(int engine);
+int rlxpp_get_engine(void);
 
 uint64_t rlxpp_n_streams(const rlxpp_t* h);
 /* 1 if the kernels with immediate multipliers serve this luxury level */

@@ -17,6 +17,8 @@ RLXPP_STREAM_MAJOR = 0
 RLXPP_INTERLEAVED = 1
 RLXPP_AOS = 0
 RLXPP_SOA = 1
+RLXPP_ENGINE_UMMA = 0
+RLXPP_ENGINE_IMAD = 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librlxpp.so")
@@ -45,6 +47,9 @@ _SIGNATURES = {
     "rlxpp_set_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     "rlxpp_multiplier": (ctypes.c_int, [ctypes.c_uint32, ctypes.c_void_p]),
     "rlxpp_seed_state": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint32, ctypes.c_void_p]),
+    "rlxpp_umma_matrix": (ctypes.c_int, [ctypes.c_uint32, ctypes.c_void_p]),
+    "rlxpp_set_engine": (ctypes.c_int, [ctypes.c_int]),
+    "rlxpp_get_engine": (ctypes.c_int, []),
     "rlxpp_n_streams": (ctypes.c_uint64, [ctypes.c_void_p]),
     "rlxpp_has_fixed_multiplier": (ctypes.c_int, [ctypes.c_uint32]),
     "rlxpp_launch_count": (ctypes.c_uint64, []),
@@ -189,6 +194,20 @@ def rlxpp_seed_state(seed: int, p: int) -> np.ndarray:
     out = np.zeros(9, np.uint64)
     _check(load().rlxpp_seed_state(seed & (2**64 - 1), p, out.ctypes.data), "rlxpp_seed_state")
     return out
+
+
+def rlxpp_umma_matrix(p: int) -> np.ndarray:
+    out = np.zeros((72, 72), np.uint8)
+    _check(load().rlxpp_umma_matrix(p, out.ctypes.data), "rlxpp_umma_matrix")
+    return out
+
+
+def rlxpp_set_engine(engine: int):
+    _check(load().rlxpp_set_engine(engine), "rlxpp_set_engine")
+
+
+def rlxpp_get_engine() -> int:
+    return int(load().rlxpp_get_engine())
 
 
 def rlxpp_n_streams(h: Handle) -> int:

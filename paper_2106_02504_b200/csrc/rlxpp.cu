@@ -15,6 +15,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -96,6 +97,16 @@ __device__ __noinline__ void exact_fold_to_ranlux(const u32* zin, u32* xout, u32
   *cout = c;
 }
 
+__device__ __noinline__ void exact_to_ranlux(const u32* xin, u32* vout, u32* cout) {
+  u32 x[18], v[18], c;
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = xin[j];
+  to_ranlux_exact(x, v, c);
+#pragma unroll
+  for (int j = 0; j < 18; j++) vout[j] = v[j];
+  *cout = c;
+}
+
 // ----------------------------------------------------------------------------- advance
 // Multiplier policy: Fixed<P> bakes A = a^P into the instruction stream; Generic carries A
 // as 18 runtime limbs (kernel parameter -> uniform registers) and runs the full-width
@@ -144,17 +155,17 @@ struct Generic {
 };
 
 // ----------------------------------------------------------------------------- kernels
-// cfg2: x <- A^reps x mod m on raw uint64[9] states, in place.
-template <class Mult, int LAYOUT>
-__global__ void __launch_bounds__(kThreads) advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
-                                                                  const __grid_constant__ Limbs18 A) {
-  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kThreads * 72 / 16 : 1];
+// Raw uint64[9] states (cfg2).  AoS: the block's 128 states are 9216 contiguous bytes: 128-bit
+// coalesced accesses to/from shared memory, each thread picks up its 72 bytes there (stride 18
+// words: 2-way bank conflict).  SoA: limb-major planes, coalesced directly.
+constexpr int kRawStageWords = kThreads * 72 / 16;
+template <int LAYOUT>
+__device__ __forceinline__ void load_raw(const u64* __restrict__ states, u64 n, uint4* stage, u32 (&x)[18]) {
   const u64 base = (u64)blockIdx.x * kThreads;
   const u64 i = base + threadIdx.x;
-  u32 x[18];
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = 0;
   if (LAYOUT == RLXPP_AOS) {
-    // the block's 128 states are 9216 contiguous bytes: 128-bit coalesced loads into shared
-    // memory, then each thread picks up its 72 bytes (stride 18 words: 2-way bank conflict)
     const u64 cnt = (n - base < (u64)kThreads ? n - base : (u64)kThreads) * 72 / 8;  // u64 words
     const uint4* src = reinterpret_cast<const uint4*>(states + base * 9);
     for (u32 q = threadIdx.x; q < (cnt + 1) / 2; q += kThreads) {
@@ -170,29 +181,19 @@ __global__ void __launch_bounds__(kThreads) advance_states_kernel(u64* __restric
 #pragma unroll
       for (int j = 0; j < 18; j++) x[j] = sw[threadIdx.x * 18 + j];
     }
-  } else {
-    if (i < n) {
+  } else if (i < n) {
 #pragma unroll
-      for (int l = 0; l < 9; l++) {
-        const u64 w = states[(u64)l * n + i];
-        x[2 * l] = (u32)w;
-        x[2 * l + 1] = (u32)(w >> 32);
-      }
+    for (int l = 0; l < 9; l++) {
+      const u64 w = states[(u64)l * n + i];
+      x[2 * l] = (u32)w;
+      x[2 * l + 1] = (u32)(w >> 32);
     }
   }
-  if (i < n) {
-    const Mult mult(A);
-    if (reps == 0) {
-      u32 z[20], r[18];
-#pragma unroll
-      for (int j = 0; j < 20; j++) z[j] = j < 18 ? x[j] : 0u;
-      exact_fold(z, r);
-#pragma unroll
-      for (int j = 0; j < 18; j++) x[j] = r[j];
-    }
-#pragma unroll 1
-    for (u32 r = 0; r < reps; r++) mult.advance(x);
-  }
+}
+template <int LAYOUT>
+__device__ __forceinline__ void store_raw(u64* __restrict__ states, u64 n, uint4* stage, const u32 (&x)[18]) {
+  const u64 base = (u64)blockIdx.x * kThreads;
+  const u64 i = base + threadIdx.x;
   if (LAYOUT == RLXPP_AOS) {
     __syncthreads();
     u32* sw = reinterpret_cast<u32*>(stage);
@@ -212,6 +213,31 @@ __global__ void __launch_bounds__(kThreads) advance_states_kernel(u64* __restric
     for (int l = 0; l < 9; l++) states[(u64)l * n + i] = (u64)x[2 * l] | ((u64)x[2 * l + 1] << 32);
   }
 }
+__device__ __forceinline__ void canonicalise(u32 (&x)[18]) {
+  u32 z[20], r[18];
+#pragma unroll
+  for (int j = 0; j < 20; j++) z[j] = j < 18 ? x[j] : 0u;
+  exact_fold(z, r);
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = r[j];
+}
+
+// cfg2: x <- A^reps x mod m on raw uint64[9] states, in place (IMAD engine).
+template <class Mult, int LAYOUT>
+__global__ void __launch_bounds__(kThreads) advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
+                                                                  const __grid_constant__ Limbs18 A) {
+  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kRawStageWords : 1];
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  u32 x[18];
+  load_raw<LAYOUT>(states, n, stage, x);
+  if (i < n) {
+    const Mult mult(A);
+    if (reps == 0) canonicalise(x);
+#pragma unroll 1
+    for (u32 r = 0; r < reps; r++) mult.advance(x);
+  }
+  store_raw<LAYOUT>(states, n, stage, x);
+}
 
 struct GenArgs {
   uint4* st;     // state planes of the whole handle
@@ -224,6 +250,7 @@ struct GenArgs {
   double* sum;   // REDUCE: per-stream outputs of this launch (already offset)
   double* sumsq;
   Limbs18 A;
+  const uint4* bmat;  // UMMA engine: shared-memory image of the byte matrix B (umma_path.cuh)
 };
 
 enum { kStoreStreamMajor = 0, kStoreInterleaved = 1, kReduce = 2 };
@@ -317,6 +344,109 @@ __global__ void __launch_bounds__(kThreads) generate_kernel(const __grid_constan
     a.sum[il] = sink.S;
     if (a.sumsq) a.sumsq[il] = sink.Q;
   }
+}
+
+}  // namespace rlx
+#include "umma_path.cuh"
+namespace rlx {
+
+// ----------------------------------------------------------------------------- UMMA engine
+// Same contract as generate_kernel / advance_states_kernel, with multiply9x9 + mod_m done by
+// the tensor core (umma_path.cuh).  One CTA = 128 streams; every thread of the CTA runs the same
+// number of issue()/collect() pairs (they contain CTA barriers), rows past `count` carry x = 0.
+__device__ __forceinline__ void to_ranlux_hot(const u32 (&x)[18], u32 (&v)[18], u32& c) {
+  u32 rare = 0;
+  to_ranlux_fast(x, v, c, rare);
+  if (__builtin_expect(rare != 0, 0)) to_ranlux_exact(x, v, c);  // inline: a call would force x, v into local memory
+}
+
+template <int MODE, bool ALIGNED>
+__global__ void __launch_bounds__(tc::kTile, 4) tc_generate_kernel(const __grid_constant__ GenArgs a) {
+  __shared__ tc::Smem smem;
+  tc::Tile tile;
+  tile.setup(smem, a.bmat);
+  const u64 il = (u64)blockIdx.x * tc::kTile + threadIdx.x;
+  const bool live = il < a.count;
+  const u64 i = a.first + il;
+  u32 x[18], v[18], pos = 12, c;
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = 0;
+  if (live) load_state(a.st, a.n_total, i, x, pos);
+  Sink<MODE> sink;
+  sink.ld = a.ld;
+  sink.S = 0.0;
+  sink.Q = 0.0;
+  sink.p = MODE == kStoreStreamMajor ? a.out + il * a.n_per : (MODE == kStoreInterleaved ? a.out + il : nullptr);
+  const u64 n = a.n_per;
+  if (ALIGNED) {
+    const u64 nblk = n / 12;
+    if (nblk > 0) tile.issue(x);
+#pragma unroll 1
+    for (u64 b = 0; b < nblk; b++) {
+      u32 z[20];
+      tile.collect(z);
+      tc::reduce_z(z, x);
+      if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
+      to_ranlux_hot(x, v, c);
+      if (live) EmitBlock<0, MODE>::all(sink, v, b * 12);
+    }
+  } else if (n > 0) {
+    const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
+    const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
+    if (pos < 12) {
+      to_ranlux_exact(x, v, c);
+      if (live) EmitBlock<0, MODE>::masked(sink, v, 0, pos, n);
+    }
+    tile.issue(x);
+#pragma unroll 1
+    for (u64 s = 1; s <= smax; s++) {
+      u32 z[20], xn[18];
+      tile.collect(z);
+      tc::reduce_z(z, xn);
+      const bool take = s <= last;  // false only at s == smax for streams that end one block early
+      if (take) {
+#pragma unroll
+        for (int j = 0; j < 18; j++) x[j] = xn[j];
+      }
+      if (s < smax) tile.issue(x);
+      if (take) {
+        to_ranlux_hot(x, v, c);
+        if (live) EmitBlock<0, MODE>::masked(sink, v, s * 12, pos, n);
+      }
+    }
+    pos = (u32)((u64)pos + n - 12 * last);
+  }
+  tile.teardown();
+  if (live) {
+    store_state(a.st, a.n_total, i, x, pos);
+    if (MODE == kReduce) {
+      a.sum[il] = sink.S;
+      if (a.sumsq) a.sumsq[il] = sink.Q;
+    }
+  }
+}
+
+template <int LAYOUT>
+__global__ void __launch_bounds__(tc::kTile, 4) tc_advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
+                                                                        const uint4* __restrict__ bmat) {
+  static_assert(tc::kTile == kThreads, "raw state I/O assumes 128 threads");
+  __shared__ tc::Smem smem;
+  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kRawStageWords : 1];
+  tc::Tile tile;
+  tile.setup(smem, bmat);
+  u32 x[18];
+  load_raw<LAYOUT>(states, n, stage, x);
+  if (reps == 0) canonicalise(x);
+  else tile.issue(x);
+#pragma unroll 1
+  for (u32 r = 0; r < reps; r++) {
+    u32 z[20];
+    tile.collect(z);
+    tc::reduce_z(z, x);
+    if (r + 1 < reps) tile.issue(x);
+  }
+  tile.teardown();
+  store_raw<LAYOUT>(states, n, stage, x);
 }
 
 // Seeding and skip-ahead ("fast exponentiation by squaring"): x <- x * prod_b T[b]^(bit b of e)
@@ -468,6 +598,46 @@ static void build_tables(uint32_t p, Tables& t, bool with_pow_tables) {
   }
 }
 
+// Shared-memory image of the byte matrix B of the UMMA engine: B[n][k] = byte n of
+// R_k = A 2^(8k) mod m (k, n < 72), zero padding up to 80 x 96, laid out as tc::b_offset says.
+static void build_bmatrix(uint32_t p, std::vector<uint8_t>& img) {
+  img.assign(tc::kBBytes, 0);
+  host::Big R = host::multiplier_ap(p);
+  for (int k = 0; k < 72; k++) {
+    uint32_t w[18];
+    R.to_u32x18(w);
+    for (int n = 0; n < 72; n++) img[tc::b_offset(n, k)] = (uint8_t)(w[n / 4] >> (8 * (n % 4)));
+    R = host::reduce(host::Big::shl(R, 8));
+  }
+}
+
+// Device copies of B, one per (device, p), kept for the life of the process (7.5 KB each).
+struct BmatEntry { int dev; uint32_t p; uint4* ptr; };
+static std::mutex g_bmat_mutex;
+static std::vector<BmatEntry> g_bmat_cache;
+static int get_bmatrix(uint32_t p, const uint4** out) {
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_bmat_mutex);
+  for (const BmatEntry& e : g_bmat_cache)
+    if (e.dev == dev && e.p == p) { *out = e.ptr; return RLXPP_OK; }
+  std::vector<uint8_t> img;
+  build_bmatrix(p, img);
+  uint4* d = nullptr;
+  CUDA_TRY(cudaMalloc(&d, tc::kBBytes));
+  cudaError_t e = cudaMemcpy(d, img.data(), tc::kBBytes, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(d);
+    return fail(RLXPP_ECUDA, "uploading the UMMA byte matrix: %s", cudaGetErrorString(e));
+  }
+  g_bmat_cache.push_back({dev, p, d});
+  *out = d;
+  return RLXPP_OK;
+}
+
+// engine used by advance_states / generate_*: the tensor-core path unless told otherwise
+static std::atomic<int> g_engine{RLXPP_ENGINE_UMMA};
+
 template <int P>
 static bool fixed_matches(const Limbs18& A) {
   for (int j = 0; j < 18; j++)
@@ -497,6 +667,7 @@ struct rlxpp {
   uint4* st = nullptr;
   uint32_t* tabA = nullptr;
   uint32_t* tabG = nullptr;
+  const uint4* bmat = nullptr;  // owned by the process-wide cache
   Tables tables;
   bool aligned = true;  // every cursor is known to be 12
   uint32_t uniform_pos = 12;
@@ -525,7 +696,22 @@ static int launch_generate_mult(const GenArgs& a, int mode, bool aligned, cudaSt
     default: return launch_generate_mode<Mult, kReduce>(a, aligned, s);
   }
 }
+template <int MODE>
+static int launch_tc_generate_mode(const GenArgs& a, bool aligned, cudaStream_t s) {
+  const unsigned grid = (unsigned)((a.count + tc::kTile - 1) / tc::kTile);
+  if (aligned) tc_generate_kernel<MODE, true><<<grid, tc::kTile, 0, s>>>(a);
+  else tc_generate_kernel<MODE, false><<<grid, tc::kTile, 0, s>>>(a);
+  LAUNCH_CHECK();
+  return RLXPP_OK;
+}
 static int launch_generate(int fixed, const GenArgs& a, int mode, bool aligned, cudaStream_t s) {
+  if (g_engine.load() == RLXPP_ENGINE_UMMA) {
+    switch (mode) {
+      case kStoreStreamMajor: return launch_tc_generate_mode<kStoreStreamMajor>(a, aligned, s);
+      case kStoreInterleaved: return launch_tc_generate_mode<kStoreInterleaved>(a, aligned, s);
+      default: return launch_tc_generate_mode<kReduce>(a, aligned, s);
+    }
+  }
 #define RLXPP_CASE(P) \
   if (fixed == P) return launch_generate_mult<Fixed<P>>(a, mode, aligned, s);
   RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
@@ -555,6 +741,14 @@ const char* rlxpp_version(void) { return "rlxpp 0.1 (sm_100a)"; }
 uint64_t rlxpp_launch_count(void) { return g_launches.load(); }
 uint64_t rlxpp_n_streams(const rlxpp_t* h) { return h ? h->n : 0; }
 
+int rlxpp_set_engine(int engine) {
+  if (engine != RLXPP_ENGINE_UMMA && engine != RLXPP_ENGINE_IMAD)
+    return fail(RLXPP_EINVAL, "rlxpp_set_engine: unknown engine %d", engine);
+  g_engine.store(engine);
+  return RLXPP_OK;
+}
+int rlxpp_get_engine(void) { return g_engine.load(); }
+
 int rlxpp_has_fixed_multiplier(uint32_t p) {
 #define RLXPP_CASE(P) \
   if (p == P) return 1;
@@ -566,6 +760,14 @@ int rlxpp_has_fixed_multiplier(uint32_t p) {
 int rlxpp_multiplier(uint32_t p, uint64_t* out_host) {
   if (!out_host || p == 0) return fail(RLXPP_EINVAL, "rlxpp_multiplier: null output or p == 0");
   host::multiplier_ap(p).to_u64x9(out_host);
+  return RLXPP_OK;
+}
+int rlxpp_umma_matrix(uint32_t p, uint8_t* out_host) {
+  if (!out_host || p == 0) return fail(RLXPP_EINVAL, "rlxpp_umma_matrix: null output or p == 0");
+  std::vector<uint8_t> img;
+  build_bmatrix(p, img);
+  for (int n = 0; n < 72; n++)
+    for (int k = 0; k < 72; k++) out_host[n * 72 + k] = img[tc::b_offset(n, k)];
   return RLXPP_OK;
 }
 int rlxpp_seed_state(uint64_t seed, uint32_t p, uint64_t* out_host) {
@@ -593,6 +795,11 @@ int rlxpp_create(rlxpp_t** hout, uint64_t n_streams, uint64_t seed, uint32_t p, 
   if (h->fixed < 0) {
     delete h;
     return fail(RLXPP_EINVAL, "rlxpp_create: rows_generated.cuh is stale for p = %u (rebuild)", p);
+  }
+  rc = get_bmatrix(p, &h->bmat);
+  if (rc) {
+    delete h;
+    return rc;
   }
   cudaError_t e = cudaMalloc(&h->st, sizeof(uint4) * 5 * n_streams);
   if (e == cudaSuccess) e = cudaMalloc(&h->tabA, 64 * 18 * sizeof(uint32_t));
@@ -672,6 +879,16 @@ int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, ui
   const int fixed = fixed_level(p, t.A);
   if (fixed < 0) return fail(RLXPP_EINVAL, "rlxpp_advance_states: rows_generated.cuh is stale for p = %u", p);
   cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (g_engine.load() == RLXPP_ENGINE_UMMA) {
+    const uint4* bmat = nullptr;
+    rc = get_bmatrix(p, &bmat);
+    if (rc) return rc;
+    const unsigned grid = (unsigned)((n_states + tc::kTile - 1) / tc::kTile);
+    if (layout == RLXPP_AOS) tc_advance_states_kernel<RLXPP_AOS><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
+    else tc_advance_states_kernel<RLXPP_SOA><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
+    LAUNCH_CHECK();
+    return RLXPP_OK;
+  }
 #define RLXPP_CASE(P) \
   if (fixed == P) return launch_advance_mult<Fixed<P>>(states_dev, n_states, reps, layout, t.A, s);
   RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
@@ -697,7 +914,7 @@ int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, i
   if ((uintptr_t)out_dev % 16) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: output must be 16-byte aligned");
   GenArgs a;
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = out_dev; a.ld = h->n;
-  a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A;
+  a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat;
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
   int rc = launch_generate(h->fixed, a, layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved, aligned,
                            h->stream);
@@ -710,7 +927,7 @@ int rlxpp_generate_reduce(rlxpp_t* h, double* sum_dev, double* sumsq_dev, uint64
   if (!h || !sum_dev) return fail(RLXPP_EINVAL, "rlxpp_generate_reduce: null argument");
   GenArgs a;
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = nullptr; a.ld = 0;
-  a.n_per = n_per_stream; a.sum = sum_dev; a.sumsq = sumsq_dev; a.A = h->tables.A;
+  a.n_per = n_per_stream; a.sum = sum_dev; a.sumsq = sumsq_dev; a.A = h->tables.A; a.bmat = h->bmat;
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
   int rc = launch_generate(h->fixed, a, kReduce, aligned, h->stream);
   if (rc) return rc;
@@ -760,7 +977,7 @@ int rlxpp_generate_doubles_host(rlxpp_t* h, double* out_host, uint64_t n_per_str
     if (done >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copy[buf], 0));  // buffer free again
     GenArgs a;
     a.st = h->st; a.n_total = h->n; a.first = first; a.count = count; a.out = h->stage[buf]; a.ld = count;
-    a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A;
+    a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat;
     rc = launch_generate(h->fixed, a, mode, aligned, h->stream);
     if (rc) return rc;
     CUDA_TRY(cudaEventRecord(h->ev_kernel[buf], h->stream));

@@ -1,0 +1,179 @@
+// Tensor-core form of the fixed-multiplier LCG advance (SURVEY f-4 "int8-limb Toeplitz
+// formulation"; BASELINE.json north_star: "Use tensor cores only if an int8-limb Toeplitz
+// formulation of the fixed-multiplier product is shown by ncu to beat the IMAD path").
+//
+// multiply9x9 + most of mod_m for a FIXED multiplier A = a^p:
+//
+//     A X  ==  sum_{k=0}^{71} xb_k R_k   (mod m),   R_k = A 2^(8k) mod m,   xb_k = byte k of X
+//
+// so with the byte matrix B[n][k] = byte n of R_k (72 x 72, host-computed for any p) the 72
+// column sums  acc_n = sum_k xb_k B[n][k] < 72 * 255^2 < 2^23  are ONE u8 x u8 -> s32 GEMM
+// tile:  D[128 streams][80] = Xbytes[128][96] * B[80][96]^T  (K padded 72 -> 96, N 72 -> 80 with
+// zeros), three tcgen05.mma.kind::i8 of K = 32 per 128 advances.  The value
+// Z = sum_n acc_n 2^(8n) < 72 * 255 * m < 2^591 is then carry-normalised per thread (one thread
+// = one TMEM lane = one stream), the 15 bits above 2^576 are folded with 2^576 == 2^240 - 1
+// (fold_fast / exact mod_m20 on the rare path) and the result is the canonical LCG state.
+//
+// Per advance and stream this replaces 324 IMAD.WIDE.U32.X (4 issue cycles each on the
+// fma-heavy pipe) by ~75 plain integer instructions.
+//
+// Protocol per CTA (128 threads = 128 streams = UMMA M = the 128 TMEM lanes), per advance:
+//   issue():   every thread stores its 72 state bytes into the K-major A tile in shared memory
+//              (generic proxy) -> fence.proxy.async -> tcgen05.fence::before_thread_sync ->
+//              __syncthreads -> thread 0: tcgen05.fence::after_thread_sync, 3 x tcgen05.mma,
+//              tcgen05.commit -> mbarrier
+//   (the threads convert and emit the PREVIOUS block's doubles while the tensor core works)
+//   collect(): mbarrier wait -> tcgen05.fence::after_thread_sync -> tcgen05.ld of 72 columns ->
+//              tcgen05.wait::ld -> normalise.
+// The next issue() orders the TMEM reads before the next MMA's TMEM writes (fence + barrier),
+// and the mbarrier wait orders the MMA's shared-memory reads before the next A-tile stores.
+#pragma once
+#include "umma.cuh"
+
+namespace rlx {
+namespace tc {
+
+constexpr int kTile = 128;                    // streams per CTA = UMMA M
+constexpr int kN = 80;                        // UMMA N (72 byte columns, padded to a multiple of 16)
+constexpr int kKChunks = 6;                   // 16-byte K chunks: 96 bytes of K = 3 MMAs of K = 32
+constexpr u32 kAChunk = kTile * 16;           // bytes of one K chunk of the A tile (16 row groups x 128 B)
+constexpr u32 kBChunk = kN * 16;              // same for B (10 row groups x 128 B)
+constexpr u32 kABytes = kKChunks * kAChunk;   // 12,288
+constexpr u32 kBBytes = kKChunks * kBChunk;   // 7,680
+constexpr u32 kTmemCols = 128;                // power of two >= kN
+constexpr u32 kIdesc = umma::idesc_u8u8_s32(kTile, kN);
+
+// Shared-memory image of B (what rlxpp_create uploads, see build_bmatrix on the host side):
+// element (n, k) at byte (k / 16) * kBChunk + (n / 8) * 128 + (n % 8) * 16 + (k % 16).
+__host__ __device__ constexpr u32 b_offset(int n, int k) {
+  return (u32)(k / 16) * kBChunk + (u32)(n / 8) * 128u + (u32)(n % 8) * 16u + (u32)(k % 16);
+}
+
+struct Smem {
+  __align__(128) uint8_t a[kABytes];
+  __align__(128) uint8_t b[kBBytes];
+  __align__(8) u64 bar;
+  u32 tmem_slot;
+};
+
+struct Tile {
+  u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of the A tile
+  u32 bar;
+  u32 phase;
+  u32 tmem;    // TMEM base address of the accumulator (lane 0, first column)
+  u32 tld;     // the same with this warp's lane quarter in bits [16,32)
+  u64 adesc, bdesc;
+
+  // CTA-collective.  bmat: device pointer to the kBBytes image of B.
+  __device__ __forceinline__ void setup(Smem& s, const uint4* __restrict__ bmat) {
+    const u32 tid = threadIdx.x;
+    uint4* sb = reinterpret_cast<uint4*>(s.b);
+    for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
+    a_row = umma::smem_u32(s.a) + tid * 16u;
+    // K bytes 80..95 of every row stay zero for the whole kernel
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a_row + 5u * kAChunk), "r"(0u) : "memory");
+    bar = umma::smem_u32(&s.bar);
+    phase = 0;
+    if (tid == 0) {
+      umma::mbar_init(bar, 1);
+      umma::fence_mbar_init();
+    }
+    if (tid < 32) umma::tmem_alloc(umma::smem_u32(&s.tmem_slot), kTmemCols);
+    umma::fence_before_sync();
+    __syncthreads();
+    umma::fence_after_sync();
+    tmem = *reinterpret_cast<volatile u32*>(&s.tmem_slot);
+    tld = tmem + (((tid >> 5) & 3u) << 21);  // lane 32 (warp % 4) in bits [16,32)
+    adesc = umma::smem_desc(umma::smem_u32(s.a), kAChunk, 128u);
+    bdesc = umma::smem_desc(umma::smem_u32(s.b), kBChunk, 128u);
+  }
+
+  // CTA-collective: start  D = Xbytes * B^T  for the 128 states x (any value < 2^576).
+  __device__ __forceinline__ void issue(const u32 (&x)[18]) {
+#pragma unroll
+    for (int g = 0; g < 4; g++)
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a_row + (u32)g * kAChunk), "r"(x[4 * g]),
+                   "r"(x[4 * g + 1]), "r"(x[4 * g + 2]), "r"(x[4 * g + 3])
+                   : "memory");
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(a_row + 4u * kAChunk), "r"(x[16]), "r"(x[17]), "r"(0u)
+                 : "memory");
+    umma::fence_proxy_async_smem();
+    umma::fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      umma::fence_after_sync();
+#pragma unroll
+      for (u32 k = 0; k < 3; k++)  // K = 32 bytes = two 16-byte chunks per MMA
+        umma::mma_i8(tmem, adesc + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
+      umma::commit(bar);
+    }
+    __syncwarp();
+  }
+
+  // Waits for the product and returns Z = sum_n acc_n 2^(8n) as 19 limbs (z[18] < 2^15).
+  __device__ __forceinline__ void collect(u32 (&z)[20]) {
+    umma::mbar_wait(bar, phase);
+    phase ^= 1u;
+    __syncwarp();
+    umma::fence_after_sync();
+    u32 c[72];
+    umma::tmem_ld72_wait(tld, c);
+    // limb k gets columns 4k .. 4k+3 at byte offsets 0, 8, 16, 24.  e_k = c0 + (c1 << 8) and
+    // o_k = c2 + (c3 << 8) are both < 2^23 + 2^31 < 2^32, so  Z = E + (O << 16)  with E, O the
+    // 18-limb numbers of limbs e_k, o_k: 36 shift-adds, 19 byte permutes, one 19-limb carry chain.
+    u32 e[18], o[18], t[19];
+#pragma unroll
+    for (int k = 0; k < 18; k++) {
+      e[k] = c[4 * k] + (c[4 * k + 1] << 8);
+      o[k] = c[4 * k + 2] + (c[4 * k + 3] << 8);
+    }
+    t[0] = o[0] << 16;
+#pragma unroll
+    for (int k = 1; k < 18; k++) t[k] = __byte_perm(o[k - 1], o[k], 0x5432);
+    t[18] = o[17] >> 16;
+    asm("add.cc.u32 %0, %19, %37;\n\t"
+        "addc.cc.u32 %1, %20, %38;\n\t"
+        "addc.cc.u32 %2, %21, %39;\n\t"
+        "addc.cc.u32 %3, %22, %40;\n\t"
+        "addc.cc.u32 %4, %23, %41;\n\t"
+        "addc.cc.u32 %5, %24, %42;\n\t"
+        "addc.cc.u32 %6, %25, %43;\n\t"
+        "addc.cc.u32 %7, %26, %44;\n\t"
+        "addc.cc.u32 %8, %27, %45;\n\t"
+        "addc.cc.u32 %9, %28, %46;\n\t"
+        "addc.cc.u32 %10, %29, %47;\n\t"
+        "addc.cc.u32 %11, %30, %48;\n\t"
+        "addc.cc.u32 %12, %31, %49;\n\t"
+        "addc.cc.u32 %13, %32, %50;\n\t"
+        "addc.cc.u32 %14, %33, %51;\n\t"
+        "addc.cc.u32 %15, %34, %52;\n\t"
+        "addc.cc.u32 %16, %35, %53;\n\t"
+        "addc.cc.u32 %17, %36, %54;\n\t"
+        "addc.u32 %18, %55, 0;"
+        : "=r"(z[0]), "=r"(z[1]), "=r"(z[2]), "=r"(z[3]), "=r"(z[4]), "=r"(z[5]), "=r"(z[6]), "=r"(z[7]), "=r"(z[8]),
+          "=r"(z[9]), "=r"(z[10]), "=r"(z[11]), "=r"(z[12]), "=r"(z[13]), "=r"(z[14]), "=r"(z[15]), "=r"(z[16]),
+          "=r"(z[17]), "=r"(z[18])
+        : "r"(e[0]), "r"(e[1]), "r"(e[2]), "r"(e[3]), "r"(e[4]), "r"(e[5]), "r"(e[6]), "r"(e[7]), "r"(e[8]), "r"(e[9]),
+          "r"(e[10]), "r"(e[11]), "r"(e[12]), "r"(e[13]), "r"(e[14]), "r"(e[15]), "r"(e[16]), "r"(e[17]), "r"(t[0]),
+          "r"(t[1]), "r"(t[2]), "r"(t[3]), "r"(t[4]), "r"(t[5]), "r"(t[6]), "r"(t[7]), "r"(t[8]), "r"(t[9]), "r"(t[10]),
+          "r"(t[11]), "r"(t[12]), "r"(t[13]), "r"(t[14]), "r"(t[15]), "r"(t[16]), "r"(t[17]), "r"(t[18]));
+    z[19] = 0;
+  }
+
+  // CTA-collective, after the last collect().
+  __device__ __forceinline__ void teardown() {
+    umma::fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) umma::tmem_dealloc(tmem, kTmemCols);
+  }
+};
+
+// x <- canonical (Z mod m) for the Z of collect()
+__device__ __forceinline__ void reduce_z(u32 (&z)[20], u32 (&x)[18]) {
+  u32 rare = 0;
+  fold_fast(z, x, rare);
+  if (__builtin_expect(rare != 0, 0)) mod_m20(z, x);  // inline: a call would force z, x into local memory
+}
+
+}  // namespace tc
+}  // namespace rlx

@@ -25,11 +25,15 @@ def torch():
     return _torch
 
 
-@pytest.fixture(scope="module")
-def rlx(torch):
+@pytest.fixture(scope="module", params=["umma", "imad"])
+def rlx(torch, request):
+    """Every parity test runs once per engine of the LCG advance (include/rlxpp.h): the tensor-core
+    path (default) and the IMAD path; both must match the oracle bit for bit."""
     import paper_2106_02504_b200 as _rlx
     _rlx.load()
-    return _rlx
+    _rlx.rlxpp_set_engine(_rlx.RLXPP_ENGINE_UMMA if request.param == "umma" else _rlx.RLXPP_ENGINE_IMAD)
+    yield _rlx
+    _rlx.rlxpp_set_engine(_rlx.RLXPP_ENGINE_UMMA)
 
 
 @pytest.fixture(scope="module")

@@ -1,0 +1,80 @@
+"""CPU tests of the C-ABI library itself: it loads, exports every symbol include/rlxpp.h declares,
+and its HOST logic (multiplier, seed state, the byte matrix of the UMMA engine) is right, checked
+against Python big integers -- not against the oracle, which shares no code with the library.
+No kernel is launched here; on a box without a GPU every compute entry point must fail loudly."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2106_02504_b200 as rlx
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+M = (1 << 576) - (1 << 240) + 1
+A1 = M - (M - 1) // (1 << 24)    # D2: a = b^-1 mod m
+
+
+def to_int(limbs):
+    return sum(int(v) << (64 * i) for i, v in enumerate(limbs))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "rlxpp.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(rlxpp_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations found in include/rlxpp.h"
+    assert declared == set(rlx.EXPORTS), declared ^ set(rlx.EXPORTS)
+    lib = rlx.load()
+    raw = ctypes.CDLL(rlx.LIB_PATH)
+    for name in declared:
+        assert hasattr(raw, name), name
+    assert lib.rlxpp_version().decode().startswith("rlxpp")
+
+
+@pytest.mark.parametrize("p", [1, 24, 389, 1024, 2048, 100])
+def test_host_multiplier_is_a_pow_p(p):
+    assert (A1 << 24) % M == 1
+    assert to_int(rlx.rlxpp_multiplier(p)) == pow(A1, p, M)
+
+
+def test_host_seed_state_is_power_of_the_multiplier():
+    for seed in (0, 1, 2, 1024, 2**64 - 1):
+        assert to_int(rlx.rlxpp_seed_state(seed, 2048)) == pow(A1, 2048 * (1 << 96) * seed, M)
+
+
+@pytest.mark.parametrize("p", [24, 389, 2048, 7])
+def test_umma_byte_matrix_reproduces_the_modular_product(p):
+    """sum_n (sum_k xb_k B[n][k]) 2^(8n) == A x (mod m), every column sum < 2^23 (so the s32
+    accumulators of tcgen05.mma kind::i8 are exact) and the total < 2^591 (one 15-bit fold)."""
+    B = rlx.rlxpp_umma_matrix(p).astype(object)
+    A = pow(A1, p, M)
+    for k in range(72):  # column k of the matrix is A 2^(8k) mod m, canonical
+        Rk = sum(int(B[n][k]) << (8 * n) for n in range(72))
+        assert Rk == (A << (8 * k)) % M
+    rng = np.random.default_rng(20210602 + p)
+    xs = [int.from_bytes(rng.bytes(72), "little") for _ in range(40)]
+    xs += [0, 1, M - 1, M, (1 << 576) - 1, M - (1 << 240), int.from_bytes(b"\xff" * 72, "little")]
+    for x in xs:
+        xb = np.array(list(x.to_bytes(72, "little")), dtype=object)
+        acc = [int(sum(int(B[n][k]) * int(xb[k]) for k in range(72))) for n in range(72)]
+        assert max(acc) < 1 << 23
+        z = sum(a << (8 * n) for n, a in enumerate(acc))
+        assert z < 1 << 591
+        assert z % M == A * x % M
+
+
+def test_engine_selection_and_errors_without_gpu():
+    assert rlx.rlxpp_get_engine() == rlx.RLXPP_ENGINE_UMMA
+    rlx.rlxpp_set_engine(rlx.RLXPP_ENGINE_IMAD)
+    assert rlx.rlxpp_get_engine() == rlx.RLXPP_ENGINE_IMAD
+    rlx.rlxpp_set_engine(rlx.RLXPP_ENGINE_UMMA)
+    with pytest.raises(rlx.RlxppError, match="unknown engine"):
+        rlx.rlxpp_set_engine(7)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_multiplier(0)
+    import torch
+    if not torch.cuda.is_available():  # no CPU fallback: creation must fail, not compute on the host
+        with pytest.raises(rlx.RlxppError):
+            rlx.rlxpp_create(16, 1, 2048, cuda_stream=0)
