@@ -16,9 +16,7 @@ Prints ONE JSON line (rank 0).  DESIGN.md "Measurement" explains every key.
 import argparse
 import json
 import os
-import subprocess
 import sys
-import tempfile
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -51,57 +49,71 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi sampling DURING the timed region (B200_PROFILING.md clocks line)."""
+    """SM clock, power and throttle reasons sampled DURING the timed region (B200_PROFILING.md clocks
+    line) through NVML in a background thread (every ~2 ms: the timed region of cfg3 is tens of ms,
+    too short for an `nvidia-smi -lms` child to start and report)."""
 
-    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
-              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
-
-    def __init__(self, gpu_index):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
-        self.proc = None
+    def __init__(self, cuda_index):
+        import threading
+        self.samples = []  # (sm_mhz, power_w, reasons bitmask)
+        self.max_mhz = None
+        self.err = None
+        self._stop = threading.Event()
+        self._thread = None
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
-                                         stdout=self.f, stderr=subprocess.DEVNULL)
-        except OSError:
-            self.proc = None
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                self.dev = pynvml.nvmlDeviceGetHandleByUUID("GPU-" + str(torch.cuda.get_device_properties(cuda_index).uuid))
+            except Exception:
+                self.dev = pynvml.nvmlDeviceGetHandleByIndex(cuda_index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM))
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        except Exception as e:  # NVML missing: the clocks object says so instead of inventing numbers
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM)
+                try:
+                    reasons = nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev)
+                except Exception:
+                    reasons = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
+                try:
+                    power = nv.nvmlDeviceGetPowerUsage(self.dev) / 1e3
+                except Exception:
+                    power = 0.0
+                self.samples.append((float(mhz), power, int(reasons)))
+            except Exception as e:
+                self.err = repr(e)
+                return
+            time.sleep(0.002)
 
     def stop(self):
-        res = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is None:
-            return res
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        self.f.flush()
-        self.f.seek(0)
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.f:
-            parts = [p.strip() for p in line.split(",")]
-            if len(parts) < 9:
-                continue
-            try:
-                sm.append(float(parts[1]))
-                mx.append(float(parts[2]))
-                pw.append(float(parts[3]))
-            except ValueError:
-                continue
-            for name, val in zip(names, parts[5:9]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        self.f.close()
-        try:
-            os.unlink(self.f.name)
-        except OSError:
-            pass
-        if sm:
-            s = sorted(sm)
-            res.update(sm_mhz=s[len(s) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm),
-                       power_w_max=max(pw))
+        res = {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0, "source": "nvml"}
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join(timeout=2)
+        if self.err:
+            res["error"] = self.err
+        if self.samples:
+            nv = self.nv
+            names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                     "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                     "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                     "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+            mask = 0
+            for _, _, r in self.samples:
+                mask |= r
+            sm = sorted(x[0] for x in self.samples)
+            res.update(sm_mhz=sm[len(sm) // 2], sm_min_mhz=sm[0], samples=len(sm),
+                       reasons=sorted(k for k, bit in names.items() if mask & bit),
+                       power_w_max=max(x[1] for x in self.samples))
         return res
 
 
@@ -173,6 +185,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--engine", default="umma", choices=["umma", "imad"],
+                    help="engine of the LCG advance (include/rlxpp.h): tensor-core GEMM (default) or IMAD.WIDE")
+    ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -196,6 +211,9 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     rlx.load()
+    engines = {"umma": rlx.RLXPP_ENGINE_UMMA, "imad": rlx.RLXPP_ENGINE_IMAD}
+    rlx.rlxpp_set_engine(engines[args.engine])
+    umma = args.engine == "umma"
 
     n_streams, n_per, p, desc = WORKLOADS[args.workload]
     first_seed = 1 + rank * n_streams  # rank g owns seeds 1 + g N .. (g + 1) N
@@ -207,7 +225,7 @@ def main():
         out = torch.empty((n_per, n_streams), dtype=torch.float64, device="cuda")
         units = n_streams * n_per
         alg_bytes = units * 8 + 2 * 80 * n_streams  # doubles written + state read and written back
-        kernel = "generate_kernel<Fixed<2048>, interleaved, aligned>"
+        kernel = "tc_generate_kernel<interleaved, aligned>" if umma else "generate_kernel<Fixed<2048>, interleaved, aligned>"
 
         def step():
             rlx.rlxpp_generate_doubles(h, out, n_per, rlx.RLXPP_INTERLEAVED)
@@ -219,7 +237,7 @@ def main():
         Q = torch.empty(n_streams, dtype=torch.float64, device="cuda")
         units = n_streams * n_per
         alg_bytes = (2 * 80 + 16) * n_streams
-        kernel = "generate_kernel<Fixed<2048>, reduce, unaligned>"
+        kernel = "tc_generate_kernel<reduce, unaligned>" if umma else "generate_kernel<Fixed<2048>, reduce, unaligned>"
 
         def step():
             rlx.rlxpp_generate_reduce(h, S, Q, n_per)
@@ -229,7 +247,7 @@ def main():
         reps = n_per
         units = n_streams * reps * 12
         alg_bytes = 144 * n_streams
-        kernel = "advance_states_kernel<Fixed<2048>, AoS>"
+        kernel = "tc_advance_states_kernel<AoS>" if umma else "advance_states_kernel<Fixed<2048>, AoS>"
 
         def step():
             rlx.rlxpp_advance_states(states, n_streams, p, reps, rlx.RLXPP_AOS)
@@ -271,17 +289,28 @@ def main():
     hbm_achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
     roof_alu = imad_nominal / IMAD_PER_DOUBLE
     roof_hbm = hbm_gbs * 1e9 / 8 if args.workload in ("cfg3", "cfg4") else float("inf")
-    roofline = {
-        "bound": "alu", "kernel": kernel, "achieved": imad_achieved / 1e9, "peak": imad_nominal / 1e9, "unit": "GIMAD/s",
-        "frac": imad_achieved / imad_nominal, "traffic": None,
-        "peak_source": f"{SM_COUNT} SMs x {IMAD_LANES_PER_CLK_SM} IMAD lanes/clk x {sm_max_mhz:.0f} MHz (DESIGN.md); "
-                       f"HBM {peak_src}",
-        "kernel_ms": kernel_ms,
-        "hbm": {"achieved": hbm_achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_achieved / hbm_gbs,
-                "algorithmic_bytes_per_launch": alg_bytes},
-        "doubles_roofline": {"alu": roof_alu, "hbm": (None if roof_hbm == float("inf") else roof_hbm),
-                             "min": min(roof_alu, roof_hbm), "frac": (units / (kernel_ms * 1e-3)) / min(roof_alu, roof_hbm)},
-    }
+    doubles_rate = units / (kernel_ms * 1e-3)
+    alu = {"achieved": imad_achieved / 1e9, "peak": imad_nominal / 1e9, "unit": "GIMAD/s", "frac": imad_achieved / imad_nominal,
+           "model": "324 products 32x32->64 per advance (27 per double) whatever the engine; peak = "
+                    f"{SM_COUNT} SMs x {IMAD_LANES_PER_CLK_SM} IMAD lanes/clk x {sm_max_mhz:.0f} MHz"}
+    hbm = {"achieved": hbm_achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_achieved / hbm_gbs,
+           "algorithmic_bytes_per_launch": alg_bytes}
+    stores = args.workload in ("cfg3", "cfg4")
+    # The bound that binds: with the UMMA engine the products run on the tensor pipe, so a workload
+    # that stores its doubles is bound by HBM writes; the IMAD engine and the store-free workloads
+    # are bound by integer issue (reported against the 324-product model, north_star).
+    if stores and umma:
+        roofline = {"bound": "hbm", "kernel": kernel, "achieved": hbm_achieved, "peak": hbm_gbs, "unit": "GB/s",
+                    "frac": hbm_achieved / hbm_gbs, "traffic": None, "peak_source": f"HBM copy {peak_src}",
+                    "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
+    else:
+        roofline = {"bound": "alu", "kernel": kernel, "achieved": alu["achieved"], "peak": alu["peak"], "unit": "GIMAD/s",
+                    "frac": alu["frac"], "traffic": None, "peak_source": alu["model"] + f" (DESIGN.md); HBM {peak_src}",
+                    "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
+    roofline["engine"] = args.engine
+    roofline["doubles_roofline"] = {"alu": roof_alu, "hbm": (None if roof_hbm == float("inf") else roof_hbm),
+                                    "min": min(roof_alu, roof_hbm), "frac": doubles_rate / min(roof_alu, roof_hbm),
+                                    "what": "north_star's roofline: the slower of nominal IMAD peak / 27 and HBM peak / 8 B"}
     if clocks.get("sm_mhz"):
         at_clock = SM_COUNT * IMAD_LANES_PER_CLK_SM * clocks["sm_mhz"] * 1e6
         roofline["frac_at_observed_clock"] = imad_achieved / at_clock
@@ -295,7 +324,24 @@ def main():
     traffic_file = os.path.join(ROOT, "profiles", "traffic_r01.json")
     if os.path.exists(traffic_file):
         with open(traffic_file) as f:
-            roofline["traffic"] = json.load(f).get(args.workload)
+            roofline["traffic"] = json.load(f).get(f"{args.workload}:{args.engine}")
+
+    # ---------------------------------------------------------------- the other engine, same workload (context)
+    compare = None
+    if not args.no_compare:
+        other = "imad" if umma else "umma"
+        rlx.rlxpp_set_engine(engines[other])
+        step()
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
+        for _ in range(3):
+            step()
+        c1.record(stream)
+        torch.cuda.synchronize()
+        compare = {"engine": other, "value": units / (c0.elapsed_time(c1) / 3 * 1e-3), "unit": UNIT, "steps": 3,
+                   "n_gpus": 1, "what": "same workload and launch configuration with the other engine, this rank only"}
+        rlx.rlxpp_set_engine(engines[args.engine])
 
     # ---------------------------------------------------------------- end to end (host buffers)
     e2e = None
@@ -354,13 +400,15 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64", "data": "synthetic",
-            "config": {"workload": args.workload, "description": desc, "n_streams_per_gpu": n_streams,
+            "dtype": ("u8 x u8 -> s32 (tcgen05.mma kind::i8) + u32 limbs -> f64" if umma
+                      else "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64"), "data": "synthetic",
+            "config": {"workload": args.workload, "engine": args.engine, "description": desc, "n_streams_per_gpu": n_streams,
                        "doubles_per_stream": n_per, "p": p, "l2": "output per step (12.9 GB) exceeds L2; no flush needed"
                        if args.workload in ("cfg3", "cfg4") else "compute-bound; working set is registers",
                        "parallelism": f"streams sharded over {world} GPU(s), no collective"},
             "lcg_advances_per_s": value / 12.0,
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "other_engine": compare,
         }
         print(json.dumps(line))
     if dist is not None:
