@@ -127,6 +127,12 @@ int rlxpp_umma_matrix(uint32_t p, uint8_t* out_host);
  * Errors: EINVAL for an unknown engine. */
 int rlxpp_set_engine(int engine);
 int rlxpp_get_engine(void);
+/* UMMA engine only.  The generate kernels run as a persistent grid over work items (128 streams x
+ * one chunk of draws); the library cuts every tile's draws into chunks so that the grid's last
+ * partial wave is short (DESIGN.md 5.1 "Scheduler").  n_chunks = 0 (default): the library decides;
+ * n_chunks > 0: every call with at least n_chunks advances per stream uses that many chunks.
+ * Results never depend on it.  Errors: EINVAL outside [0, 4096]. */
+int rlxpp_set_chunks(int n_chunks);
 
 uint64_t rlxpp_n_streams(const rlxpp_t* h);
 /* 1 if the kernels with immediate multipliers serve this luxury level */

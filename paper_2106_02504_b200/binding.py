@@ -50,6 +50,7 @@ _SIGNATURES = {
     "rlxpp_umma_matrix": (ctypes.c_int, [ctypes.c_uint32, ctypes.c_void_p]),
     "rlxpp_set_engine": (ctypes.c_int, [ctypes.c_int]),
     "rlxpp_get_engine": (ctypes.c_int, []),
+    "rlxpp_set_chunks": (ctypes.c_int, [ctypes.c_int]),
     "rlxpp_n_streams": (ctypes.c_uint64, [ctypes.c_void_p]),
     "rlxpp_has_fixed_multiplier": (ctypes.c_int, [ctypes.c_uint32]),
     "rlxpp_launch_count": (ctypes.c_uint64, []),
@@ -204,6 +205,10 @@ def rlxpp_umma_matrix(p: int) -> np.ndarray:
 
 def rlxpp_set_engine(engine: int):
     _check(load().rlxpp_set_engine(engine), "rlxpp_set_engine")
+
+
+def rlxpp_set_chunks(n_chunks: int):
+    _check(load().rlxpp_set_chunks(n_chunks), "rlxpp_set_chunks")
 
 
 def rlxpp_get_engine() -> int:

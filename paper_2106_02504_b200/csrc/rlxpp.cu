@@ -61,10 +61,10 @@ constexpr int kThreads = 128;
 __device__ __forceinline__ void load_state(const uint4* __restrict__ st, u64 n, u64 i, u32 (&x)[18], u32& pos) {
 #pragma unroll
   for (int g = 0; g < 4; g++) {
-    const uint4 q = st[(u64)g * n + i];
+    const uint4 q = __ldcg(st + (u64)g * n + i);  // L2: another CTA may have written it (chunked items)
     x[4 * g] = q.x; x[4 * g + 1] = q.y; x[4 * g + 2] = q.z; x[4 * g + 3] = q.w;
   }
-  const uint4 q = st[4 * n + i];
+  const uint4 q = __ldcg(st + 4 * n + i);
   x[16] = q.x; x[17] = q.y; pos = q.z;
 }
 __device__ __forceinline__ void store_state(uint4* __restrict__ st, u64 n, u64 i, const u32 (&x)[18], u32 pos) {
@@ -251,6 +251,10 @@ struct GenArgs {
   double* sumsq;
   Limbs18 A;
   const uint4* bmat;  // UMMA engine: shared-memory image of the byte matrix B (umma_path.cuh)
+  // UMMA engine, persistent scheduler: sched[0] = ticket counter, sched[1 + tile] = finished chunks
+  u32* sched;
+  u32 n_tiles, n_chunks;
+  u64 chunk_len;      // draws per chunk (a multiple of 12 when n_chunks > 1)
 };
 
 enum { kStoreStreamMajor = 0, kStoreInterleaved = 1, kReduce = 2 };
@@ -360,79 +364,117 @@ __device__ __forceinline__ void to_ranlux_hot(const u32 (&x)[18], u32 (&v)[18], 
   if (__builtin_expect(rare != 0, 0)) to_ranlux_exact(x, v, c);  // inline: a call would force x, v into local memory
 }
 
+// Persistent grid with a ticket scheduler.  A work item = (tile of 128 streams, chunk of
+// chunk_len draws); ticket w is item (w % n_tiles, w / n_tiles), so the chunks of one tile are
+// handed out in order and sched[1 + tile] counts the chunks of it that are finished (state written
+// back).  With n_chunks == 1 this is a plain grid-stride loop over tiles; with more, the grid's last
+// partial wave shrinks from a whole tile's work to one chunk's (cfg4 / cfg5: 2,048 tiles over
+// 148 x 5 CTAs).  A CTA that waits for chunk c - 1 of its tile waits for an EARLIER ticket, which a
+// resident CTA holds: no deadlock whatever the number of resident CTAs.
 template <int MODE, bool ALIGNED>
-__global__ void __launch_bounds__(tc::kTile, 4) tc_generate_kernel(const __grid_constant__ GenArgs a) {
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(const __grid_constant__ GenArgs a) {
   __shared__ tc::Smem smem;
-  tc::Tile tile;
+  tc::Tile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
   tile.setup(smem, a.bmat);
-  const u64 il = (u64)blockIdx.x * tc::kTile + threadIdx.x;
-  const bool live = il < a.count;
-  const u64 i = a.first + il;
-  u32 x[18], v[18], pos = 12, c;
-#pragma unroll
-  for (int j = 0; j < 18; j++) x[j] = 0;
-  if (live) load_state(a.st, a.n_total, i, x, pos);
-  Sink<MODE> sink;
-  sink.ld = a.ld;
-  sink.S = 0.0;
-  sink.Q = 0.0;
-  sink.p = MODE == kStoreStreamMajor ? a.out + il * a.n_per : (MODE == kStoreInterleaved ? a.out + il : nullptr);
-  const u64 n = a.n_per;
-  if (ALIGNED) {
-    const u64 nblk = n / 12;
-    if (nblk > 0) tile.issue(x);
-#pragma unroll 1
-    for (u64 b = 0; b < nblk; b++) {
-      u32 z[20];
-      tile.collect(z);
-      tc::reduce_z(z, x);
-      if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
-      to_ranlux_hot(x, v, c);
-      if (live) EmitBlock<0, MODE>::all(sink, v, b * 12);
-    }
-  } else if (n > 0) {
-    const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
-    const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
-    if (pos < 12) {
-      to_ranlux_exact(x, v, c);
-      if (live) EmitBlock<0, MODE>::masked(sink, v, 0, pos, n);
-    }
-    tile.issue(x);
-#pragma unroll 1
-    for (u64 s = 1; s <= smax; s++) {
-      u32 z[20], xn[18];
-      tile.collect(z);
-      tc::reduce_z(z, xn);
-      const bool take = s <= last;  // false only at s == smax for streams that end one block early
-      if (take) {
-#pragma unroll
-        for (int j = 0; j < 18; j++) x[j] = xn[j];
+  const u64 n_items = (u64)a.n_tiles * a.n_chunks;
+  for (;;) {
+    if (threadIdx.x == 0) smem.ticket = atomicAdd(a.sched, 1u);
+    __syncthreads();
+    const u64 w = smem.ticket;
+    if (w >= n_items) break;
+    const u32 tidx = (u32)(w % a.n_tiles), chunk = (u32)(w / a.n_tiles);
+    if (chunk > 0) {
+      if (threadIdx.x == 0) {
+        u32 done;
+        do {
+          asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(a.sched + 1 + tidx) : "memory");
+        } while (done < chunk);
       }
-      if (s < smax) tile.issue(x);
-      if (take) {
+      __syncthreads();
+    }
+    const u64 il = (u64)tidx * tc::kTile + threadIdx.x;
+    const bool live = il < a.count;
+    const u64 i = a.first + il;
+    const u64 t0 = (u64)chunk * a.chunk_len;                               // first draw of this item
+    const u64 n = a.n_per - t0 < a.chunk_len ? a.n_per - t0 : a.chunk_len;  // its draws
+    u32 x[18], v[18], pos = 12, c;
+#pragma unroll
+    for (int j = 0; j < 18; j++) x[j] = 0;
+    if (live) load_state(a.st, a.n_total, i, x, pos);
+    Sink<MODE> sink;
+    sink.ld = a.ld;
+    sink.S = 0.0;
+    sink.Q = 0.0;
+    if (MODE == kReduce && chunk > 0 && live) {
+      sink.S = __ldcg(a.sum + il);
+      sink.Q = __ldcg(a.sumsq + il);
+    }
+    sink.p = MODE == kStoreStreamMajor ? a.out + il * a.n_per + t0
+                                       : (MODE == kStoreInterleaved ? a.out + il + t0 * a.ld : nullptr);
+    if (ALIGNED) {
+      const u64 nblk = n / 12;
+      if (nblk > 0) tile.issue(x);
+#pragma unroll 1
+      for (u64 b = 0; b < nblk; b++) {
+        u32 z[20];
+        tile.collect(z);
+        tc::reduce_z(z, x);
+        if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
         to_ranlux_hot(x, v, c);
-        if (live) EmitBlock<0, MODE>::masked(sink, v, s * 12, pos, n);
+        if (live) EmitBlock<0, MODE>::all(sink, v, b * 12);
+      }
+    } else if (n > 0) {
+      const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
+      const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
+      if (pos < 12) {
+        to_ranlux_exact(x, v, c);
+        if (live) EmitBlock<0, MODE>::masked(sink, v, 0, pos, n);
+      }
+      tile.issue(x);
+#pragma unroll 1
+      for (u64 s = 1; s <= smax; s++) {
+        u32 z[20], xn[18];
+        tile.collect(z);
+        tc::reduce_z(z, xn);
+        const bool take = s <= last;  // false only at s == smax for streams that end one block early
+        if (take) {
+#pragma unroll
+          for (int j = 0; j < 18; j++) x[j] = xn[j];
+        }
+        if (s < smax) tile.issue(x);
+        if (take) {
+          to_ranlux_hot(x, v, c);
+          if (live) EmitBlock<0, MODE>::masked(sink, v, s * 12, pos, n);
+        }
+      }
+      pos = (u32)((u64)pos + n - 12 * last);
+    }
+    if (live) {
+      store_state(a.st, a.n_total, i, x, pos);
+      if (MODE == kReduce) {
+        a.sum[il] = sink.S;
+        if (a.sumsq) a.sumsq[il] = sink.Q;
       }
     }
-    pos = (u32)((u64)pos + n - 12 * last);
+    if (a.n_chunks > 1) {  // publish: state (and partial sums) of this tile are in global memory
+      __threadfence();
+      __syncthreads();
+      if (threadIdx.x == 0)
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.sched + 1 + tidx), "r"(chunk + 1u) : "memory");
+    } else {
+      __syncthreads();  // smem.ticket is rewritten at the top of the loop
+    }
   }
   tile.teardown();
-  if (live) {
-    store_state(a.st, a.n_total, i, x, pos);
-    if (MODE == kReduce) {
-      a.sum[il] = sink.S;
-      if (a.sumsq) a.sumsq[il] = sink.Q;
-    }
-  }
 }
 
 template <int LAYOUT>
-__global__ void __launch_bounds__(tc::kTile, 4) tc_advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
                                                                         const uint4* __restrict__ bmat) {
   static_assert(tc::kTile == kThreads, "raw state I/O assumes 128 threads");
   __shared__ tc::Smem smem;
   __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kRawStageWords : 1];
-  tc::Tile tile;
+  tc::Tile<tc::kSyncArrive> tile;
   tile.setup(smem, bmat);
   u32 x[18];
   load_raw<LAYOUT>(states, n, stage, x);
@@ -637,6 +679,8 @@ static int get_bmatrix(uint32_t p, const uint4** out) {
 
 // engine used by advance_states / generate_*: the tensor-core path unless told otherwise
 static std::atomic<int> g_engine{RLXPP_ENGINE_UMMA};
+// > 0: cut every tile into this many chunks whatever plan_items says (rlxpp_set_chunks; tests)
+static std::atomic<int> g_force_chunks{0};
 
 template <int P>
 static bool fixed_matches(const Limbs18& A) {
@@ -668,6 +712,8 @@ struct rlxpp {
   uint32_t* tabA = nullptr;
   uint32_t* tabG = nullptr;
   const uint4* bmat = nullptr;  // owned by the process-wide cache
+  uint32_t* sched = nullptr;    // scheduler words of the persistent UMMA kernel: 1 + ceil(n / 128)
+  double* scratch_q = nullptr;  // sum of squares when the caller passes none (chunked reduce carries it)
   Tables tables;
   bool aligned = true;  // every cursor is known to be 12
   uint32_t uniform_pos = 12;
@@ -696,9 +742,52 @@ static int launch_generate_mult(const GenArgs& a, int mode, bool aligned, cudaSt
     default: return launch_generate_mode<Mult, kReduce>(a, aligned, s);
   }
 }
+// Work items of the persistent UMMA kernel: how many chunks to cut every tile's n_per draws into so
+// that the last, partial wave of the grid is short.  One chunk unless the tiles alone fill the
+// resident CTAs badly; a chunk is never shorter than 16 advances (state I/O and pipeline fill).
+static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_t* n_chunks, uint64_t* chunk_len) {
+  *n_chunks = 1;
+  *chunk_len = n_per;
+  const uint64_t blocks = n_per / 12;
+  if (n_tiles <= slots || blocks < 32) return;
+  double best = 0.0;
+  uint64_t best_c = 1;
+  for (uint64_t c = 1; c <= 16 && blocks / c >= 16; c++) {
+    const uint64_t items = n_tiles * c, waves = (items + slots - 1) / slots;
+    const double eff = (double)items / (double)(waves * slots);
+    if (eff > best + 1e-9) { best = eff; best_c = c; }
+    if (eff >= 0.97) break;
+  }
+  if (best_c == 1) return;
+  const uint64_t len = (blocks + best_c - 1) / best_c * 12;
+  *chunk_len = len;
+  *n_chunks = (uint32_t)((n_per + len - 1) / len);
+}
+
+static unsigned tc_slots() {
+  static unsigned slots = 0;
+  if (slots == 0) {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    slots = (unsigned)sms * tc::kCtasPerSm;
+  }
+  return slots;
+}
+
 template <int MODE>
-static int launch_tc_generate_mode(const GenArgs& a, bool aligned, cudaStream_t s) {
-  const unsigned grid = (unsigned)((a.count + tc::kTile - 1) / tc::kTile);
+static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
+  const uint64_t n_tiles = (a.count + tc::kTile - 1) / tc::kTile;
+  const unsigned slots = tc_slots();
+  a.n_tiles = (u32)n_tiles;
+  plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len);
+  if (g_force_chunks.load() > 0 && a.n_per / 12 >= (uint64_t)g_force_chunks.load()) {  // test hook
+    const uint64_t c = (uint64_t)g_force_chunks.load(), blocks = a.n_per / 12;
+    a.chunk_len = (blocks + c - 1) / c * 12;
+    a.n_chunks = (u32)((a.n_per + a.chunk_len - 1) / a.chunk_len);
+  }
+  const uint64_t items = n_tiles * a.n_chunks;
+  const unsigned grid = (unsigned)(items < slots ? items : slots);
+  CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
   if (aligned) tc_generate_kernel<MODE, true><<<grid, tc::kTile, 0, s>>>(a);
   else tc_generate_kernel<MODE, false><<<grid, tc::kTile, 0, s>>>(a);
   LAUNCH_CHECK();
@@ -748,6 +837,11 @@ int rlxpp_set_engine(int engine) {
   return RLXPP_OK;
 }
 int rlxpp_get_engine(void) { return g_engine.load(); }
+int rlxpp_set_chunks(int n_chunks) {
+  if (n_chunks < 0 || n_chunks > 4096) return fail(RLXPP_EINVAL, "rlxpp_set_chunks: %d not in [0, 4096]", n_chunks);
+  g_force_chunks.store(n_chunks);
+  return RLXPP_OK;
+}
 
 int rlxpp_has_fixed_multiplier(uint32_t p) {
 #define RLXPP_CASE(P) \
@@ -802,6 +896,7 @@ int rlxpp_create(rlxpp_t** hout, uint64_t n_streams, uint64_t seed, uint32_t p, 
     return rc;
   }
   cudaError_t e = cudaMalloc(&h->st, sizeof(uint4) * 5 * n_streams);
+  if (e == cudaSuccess) e = cudaMalloc(&h->sched, sizeof(uint32_t) * (1 + (n_streams + tc::kTile - 1) / tc::kTile));
   if (e == cudaSuccess) e = cudaMalloc(&h->tabA, 64 * 18 * sizeof(uint32_t));
   if (e == cudaSuccess) e = cudaMalloc(&h->tabG, 64 * 18 * sizeof(uint32_t));
   if (e == cudaSuccess)
@@ -830,6 +925,8 @@ int rlxpp_destroy(rlxpp_t* h) {
   if (!h) return RLXPP_OK;
   if (h->stream || h->st) cudaStreamSynchronize(h->stream);
   cudaFree(h->st);
+  cudaFree(h->sched);
+  cudaFree(h->scratch_q);
   cudaFree(h->tabA);
   cudaFree(h->tabG);
   for (int b = 0; b < 2; b++) {
@@ -914,7 +1011,7 @@ int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, i
   if ((uintptr_t)out_dev % 16) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: output must be 16-byte aligned");
   GenArgs a;
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = out_dev; a.ld = h->n;
-  a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat;
+  a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
   int rc = launch_generate(h->fixed, a, layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved, aligned,
                            h->stream);
@@ -925,9 +1022,13 @@ int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, i
 
 int rlxpp_generate_reduce(rlxpp_t* h, double* sum_dev, double* sumsq_dev, uint64_t n_per_stream) {
   if (!h || !sum_dev) return fail(RLXPP_EINVAL, "rlxpp_generate_reduce: null argument");
+  if (!sumsq_dev && g_engine.load() == RLXPP_ENGINE_UMMA) {
+    if (!h->scratch_q) CUDA_TRY(cudaMalloc(&h->scratch_q, sizeof(double) * h->n));
+    sumsq_dev = h->scratch_q;
+  }
   GenArgs a;
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = nullptr; a.ld = 0;
-  a.n_per = n_per_stream; a.sum = sum_dev; a.sumsq = sumsq_dev; a.A = h->tables.A; a.bmat = h->bmat;
+  a.n_per = n_per_stream; a.sum = sum_dev; a.sumsq = sumsq_dev; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
   int rc = launch_generate(h->fixed, a, kReduce, aligned, h->stream);
   if (rc) return rc;
@@ -977,7 +1078,7 @@ int rlxpp_generate_doubles_host(rlxpp_t* h, double* out_host, uint64_t n_per_str
     if (done >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copy[buf], 0));  // buffer free again
     GenArgs a;
     a.st = h->st; a.n_total = h->n; a.first = first; a.count = count; a.out = h->stage[buf]; a.ld = count;
-    a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat;
+    a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
     rc = launch_generate(h->fixed, a, mode, aligned, h->stream);
     if (rc) return rc;
     CUDA_TRY(cudaEventRecord(h->ev_kernel[buf], h->stream));

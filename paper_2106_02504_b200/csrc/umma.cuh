@@ -73,6 +73,9 @@ __device__ __forceinline__ void mbar_wait(u32 bar, u32 parity) {
 // Tensor memory: whole-warp calls.  ncols: power of two >= 32.  The base address is written to smem.
 __device__ __forceinline__ void tmem_alloc(u32 smem_dst, u32 ncols) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+}
+// after the CTA's last allocation
+__device__ __forceinline__ void tmem_relinquish() {
   asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void tmem_dealloc(u32 taddr, u32 ncols) {
@@ -84,7 +87,8 @@ __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.
 // 32-bit columns starting at the column in taddr (lane in bits [16,32), column in bits [0,16)).
 // All 72 accumulator columns of this thread's TMEM lane, then tcgen05.wait::ld -- ONE asm block, so
 // that no use of the registers can be scheduled before the wait.
-__device__ __forceinline__ void tmem_ld72_wait(u32 taddr, u32 (&r)[72]) {
+// taddr_lo: columns 0..63, taddr_hi: columns 64..71 (they may sit in different allocations).
+__device__ __forceinline__ void tmem_ld72_wait(u32 taddr_lo, u32 taddr_hi, u32 (&r)[72]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x64.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32, %33, %34, %35, %36, %37, %38, %39, %40, %41, %42, %43, %44, %45, %46, %47, %48, %49, %50, %51, %52, %53, %54, %55, %56, %57, %58, %59, %60, %61, %62, %63}, [%72];\n\t"
       "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%64, %65, %66, %67, %68, %69, %70, %71}, [%73];\n\t"
@@ -98,7 +102,7 @@ __device__ __forceinline__ void tmem_ld72_wait(u32 taddr, u32 (&r)[72]) {
         "=r"(r[48]), "=r"(r[49]), "=r"(r[50]), "=r"(r[51]), "=r"(r[52]), "=r"(r[53]), "=r"(r[54]), "=r"(r[55]), 
         "=r"(r[56]), "=r"(r[57]), "=r"(r[58]), "=r"(r[59]), "=r"(r[60]), "=r"(r[61]), "=r"(r[62]), "=r"(r[63]), 
         "=r"(r[64]), "=r"(r[65]), "=r"(r[66]), "=r"(r[67]), "=r"(r[68]), "=r"(r[69]), "=r"(r[70]), "=r"(r[71])
-      : "r"(taddr), "r"(taddr + 64u)
+      : "r"(taddr_lo), "r"(taddr_hi)
       : "memory");
 }
 

@@ -41,7 +41,18 @@ constexpr u32 kBChunk = kN * 16;              // same for B (10 row groups x 128
 constexpr u32 kABytes = kKChunks * kAChunk;   // 12,288
 constexpr u32 kBBytes = kKChunks * kBChunk;   // 7,680
 constexpr u32 kTmemCols = 128;                // power of two >= kN
+constexpr int kCtasPerSm = 4;                 // 4 x 128 = the SM's 512 TMEM columns
 constexpr u32 kIdesc = umma::idesc_u8u8_s32(kTile, kN);
+
+// How the CTA hands the freshly written A tile to the thread that issues the MMAs.
+//   kSyncCta:    __syncthreads, warp 0 issues.  Every warp waits for the slowest one.
+//   kSyncArrive: named barrier 1 -- three warps `bar.arrive` and go straight on to their doubles, only the
+//                issuing warp `bar.sync`s (asleep, no polling).  The issuing warp is rotated over the
+//                SM's co-resident CTAs (warp w always runs on scheduler w % 4; the TMEM column base
+//                0 / 128 / 256 / 384 is unique per resident CTA), so the four schedulers share the
+//                issue work.  Measured (profiles/ab_r01_sync.md): +14 % on the store kernels, +5 % on
+//                the raw advance, -6 % on the fused reduce, which therefore keeps kSyncCta.
+enum { kSyncCta = 0, kSyncArrive = 2 };
 
 // Shared-memory image of B (what rlxpp_create uploads, see build_bmatrix on the host side):
 // element (n, k) at byte (k / 16) * kBChunk + (n / 8) * 128 + (n % 8) * 16 + (k % 16).
@@ -52,16 +63,19 @@ __host__ __device__ constexpr u32 b_offset(int n, int k) {
 struct Smem {
   __align__(128) uint8_t a[kABytes];
   __align__(128) uint8_t b[kBBytes];
-  __align__(8) u64 bar;
+  __align__(8) u64 bar;        // MMA done (tcgen05.commit)
   u32 tmem_slot;
+  u32 ticket;                  // work item of the persistent scheduler (rlxpp.cu)
 };
 
+template <int SYNC>
 struct Tile {
   u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of the A tile
   u32 bar;
   u32 phase;
   u32 tmem;    // TMEM base address of the accumulator (lane 0, first column)
   u32 tld;     // the same with this warp's lane quarter in bits [16,32)
+  u32 issuer;         // the warp that issues this CTA's MMAs
   u64 adesc, bdesc;
 
   // CTA-collective.  bmat: device pointer to the kBBytes image of B.
@@ -78,11 +92,15 @@ struct Tile {
       umma::mbar_init(bar, 1);
       umma::fence_mbar_init();
     }
-    if (tid < 32) umma::tmem_alloc(umma::smem_u32(&s.tmem_slot), kTmemCols);
+    if (tid < 32) {
+      umma::tmem_alloc(umma::smem_u32(&s.tmem_slot), kTmemCols);
+      umma::tmem_relinquish();
+    }
     umma::fence_before_sync();
     __syncthreads();
     umma::fence_after_sync();
     tmem = *reinterpret_cast<volatile u32*>(&s.tmem_slot);
+    issuer = SYNC == kSyncArrive ? ((tmem & 0xFFFFu) / kTmemCols) & 3u : 0u;
     tld = tmem + (((tid >> 5) & 3u) << 21);  // lane 32 (warp % 4) in bits [16,32)
     adesc = umma::smem_desc(umma::smem_u32(s.a), kAChunk, 128u);
     bdesc = umma::smem_desc(umma::smem_u32(s.b), kBChunk, 128u);
@@ -99,15 +117,28 @@ struct Tile {
                  : "memory");
     umma::fence_proxy_async_smem();
     umma::fence_before_sync();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      umma::fence_after_sync();
-#pragma unroll
-      for (u32 k = 0; k < 3; k++)  // K = 32 bytes = two 16-byte chunks per MMA
-        umma::mma_i8(tmem, adesc + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
-      umma::commit(bar);
+    if (SYNC == kSyncArrive) {
+      if ((threadIdx.x >> 5) == issuer) {
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if ((threadIdx.x & 31u) == 0) issue_mma();
+        __syncwarp();
+      } else {
+        asm volatile("bar.arrive 1, 128;" ::: "memory");
+      }
+    } else {
+      __syncthreads();
+      if (threadIdx.x == 0) issue_mma();
+      __syncwarp();
     }
-    __syncwarp();
+  }
+
+  // One thread: D = Xbytes * B^T as three K steps of 32 bytes (two 16-byte chunks each).
+  __device__ __forceinline__ void issue_mma() {
+    umma::fence_after_sync();
+#pragma unroll
+    for (u32 k = 0; k < 3; k++)
+      umma::mma_i8(tmem, adesc + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
+    umma::commit(bar);
   }
 
   // Waits for the product and returns Z = sum_n acc_n 2^(8n) as 19 limbs (z[18] < 2^15).
@@ -117,7 +148,7 @@ struct Tile {
     __syncwarp();
     umma::fence_after_sync();
     u32 c[72];
-    umma::tmem_ld72_wait(tld, c);
+    umma::tmem_ld72_wait(tld, tld + 64u, c);
     // limb k gets columns 4k .. 4k+3 at byte offsets 0, 8, 16, 24.  e_k = c0 + (c1 << 8) and
     // o_k = c2 + (c3 << 8) are both < 2^23 + 2^31 < 2^32, so  Z = E + (O << 16)  with E, O the
     // 18-limb numbers of limbs e_k, o_k: 36 shift-adds, 19 byte permutes, one 19-limb carry chain.

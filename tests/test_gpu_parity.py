@@ -311,6 +311,54 @@ def test_unaligned_interleaved_and_reduce_after_per_stream_skips(rlx, torch, ora
     assert_bits_equal(s.cpu().numpy(), want, "reduce after unaligned draws")
 
 
+@pytest.mark.parametrize("n_chunks", [2, 3, 7])
+def test_chunked_work_items_give_the_same_results(rlx, torch, oracle, nthreads, n_chunks):
+    """UMMA engine: the persistent kernel cuts a tile's draws into chunks handed to different CTAs
+    (rlxpp_set_chunks forces it at a small size; cfg4 / cfg5 full size use it by default).  State,
+    cursor and partial sums travel through global memory between chunks: results must not change.
+    More tiles (41) than fit a chunk-major order by accident, ragged last tile, ragged last chunk."""
+    n, per = 41 * 128 - 29, 12 * 50
+    dist = inputs.splitmix64(4242, n) % np.uint64(1000)
+    rlx.rlxpp_set_chunks(n_chunks)
+    try:
+        # aligned cursors, both store layouts
+        h = rlx.rlxpp_create(n, 9, 2048)
+        a = torch.empty((n, per), dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_doubles(h, a, per, rlx.RLXPP_STREAM_MAJOR)
+        b = torch.empty((per, n), dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_doubles(h, b, per, rlx.RLXPP_INTERLEAVED)
+        ref = oracle.streams(inputs.seeds(n, 9), 2048, 2 * per, want=("doubles", "state"), nthreads=nthreads)
+        assert_bits_equal(a.cpu().numpy(), ref["doubles"][:, :per], "chunked stream-major")
+        assert_bits_equal(b.cpu().numpy().T, ref["doubles"][:, per:], "chunked interleaved")
+        check_state(rlx, torch, h, ref, "chunked aligned")
+        rlx.rlxpp_destroy(h)
+        # per-stream cursors, draw count not a multiple of 12, fused sums carried across chunks
+        per2 = per + 5
+        h = rlx.rlxpp_create(n, 9, 2048)
+        rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+        s = torch.empty(n, dtype=torch.float64, device="cuda")
+        q = torch.empty(n, dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_reduce(h, s, q, per2)
+        c = torch.empty((per2, n), dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_doubles(h, c, per2, rlx.RLXPP_INTERLEAVED)
+        s2 = torch.empty(n, dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_reduce(h, s2, None, per2)  # no sum of squares: library scratch carries it
+        torch.cuda.synchronize()
+        ref = oracle.streams(inputs.seeds(n, 9), 2048, per2, skips=dist, want=("sums",), nthreads=nthreads)
+        assert_bits_equal(s.cpu().numpy(), ref["sum"], "chunked sum")
+        assert_bits_equal(q.cpu().numpy(), ref["sumsq"], "chunked sum of squares")
+        ref = oracle.streams(inputs.seeds(n, 9), 2048, 3 * per2, skips=dist, want=("doubles", "state"), nthreads=nthreads)
+        assert_bits_equal(c.cpu().numpy().T, ref["doubles"][:, per2:2 * per2], "chunked unaligned interleaved")
+        want = np.zeros(n)
+        for t in range(2 * per2, 3 * per2):
+            want = want + ref["doubles"][:, t]
+        assert_bits_equal(s2.cpu().numpy(), want, "chunked sum without sumsq")
+        check_state(rlx, torch, h, ref, "chunked unaligned")
+        rlx.rlxpp_destroy(h)
+    finally:
+        rlx.rlxpp_set_chunks(0)
+
+
 def test_generic_multiplier_streams(rlx, torch, oracle, nthreads):
     """A luxury level without baked-in rows (p = 100) runs the full multiply9x9 + mod_m kernels."""
     assert not rlx.rlxpp_has_fixed_multiplier(100)
