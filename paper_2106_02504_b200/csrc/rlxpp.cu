@@ -273,9 +273,10 @@ struct Sink {
 
 template <int J, int MODE>
 struct EmitBlock {
-  // all 12 draws of block v go to output indices t0 .. t0 + 11
+  // all 12 draws of block v go to output indices t0 .. t0 + 11 (VEC: t0 is even and p is 16-byte aligned)
+  template <bool VEC = true>
   static __device__ __forceinline__ void all(Sink<MODE>& s, const u32 (&v)[18], u64 t0) {
-    if (MODE == kStoreStreamMajor) {
+    if (MODE == kStoreStreamMajor && VEC) {
       if (J % 2 == 0) {  // two draws per 128-bit store (p + t0 is 16-byte aligned: n_per % 12 == 0)
         double2 d2 = make_double2(draw_double<J>(v), draw_double<J + 1>(v));
         __stcs(reinterpret_cast<double2*>(s.p + t0 + J), d2);
@@ -283,7 +284,7 @@ struct EmitBlock {
     } else {
       s.emit(t0 + J, draw_double<J>(v));
     }
-    EmitBlock<J + 1, MODE>::all(s, v, t0);
+    EmitBlock<J + 1, MODE>::template all<VEC>(s, v, t0);
   }
   // draw J of the block at absolute draw position q0 + J is output index q0 + J - pos if in [0, n)
   static __device__ __forceinline__ void masked(Sink<MODE>& s, const u32 (&v)[18], u64 q0, u32 pos, u64 n) {
@@ -297,6 +298,7 @@ struct EmitBlock {
 };
 template <int MODE>
 struct EmitBlock<12, MODE> {
+  template <bool VEC = true>
   static __device__ __forceinline__ void all(Sink<MODE>&, const u32 (&)[18], u64) {}
   static __device__ __forceinline__ void masked(Sink<MODE>&, const u32 (&)[18], u64, u32, u64) {}
 };
@@ -431,8 +433,19 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         if (live) EmitBlock<0, MODE>::masked(sink, v, 0, pos, n);
       }
       tile.issue(x);
+      // blocks 1 .. smax - 2 lie wholly inside [0, n) for every cursor (last >= smax - 1): no masks
+      u64 s = 1;
 #pragma unroll 1
-      for (u64 s = 1; s <= smax; s++) {
+      for (; s + 2 <= smax; s++) {
+        u32 z[20];
+        tile.collect(z);
+        tc::reduce_z(z, x);
+        tile.issue(x);
+        to_ranlux_hot(x, v, c);
+        if (live) EmitBlock<0, MODE>::template all<false>(sink, v, s * 12 - pos);
+      }
+#pragma unroll 1
+      for (; s <= smax; s++) {
         u32 z[20], xn[18];
         tile.collect(z);
         tc::reduce_z(z, xn);
