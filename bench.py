@@ -187,6 +187,8 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--engine", default="umma", choices=["umma", "imad"],
                     help="engine of the LCG advance (include/rlxpp.h): tensor-core GEMM (default) or IMAD.WIDE")
+    ap.add_argument("--layout", default="interleaved", choices=["interleaved", "stream_major"],
+                    help="cfg3 / cfg4 output layout (BASELINE cfg3 names the interleaved one; stream_major is context)")
     ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
@@ -225,10 +227,12 @@ def main():
         out = torch.empty((n_per, n_streams), dtype=torch.float64, device="cuda")
         units = n_streams * n_per
         alg_bytes = units * 8 + 2 * 80 * n_streams  # doubles written + state read and written back
-        kernel = "tc_generate_kernel<interleaved, aligned>" if umma else "generate_kernel<Fixed<2048>, interleaved, aligned>"
+        lay = rlx.RLXPP_INTERLEAVED if args.layout == "interleaved" else rlx.RLXPP_STREAM_MAJOR
+        kernel = (f"tc_generate_kernel<{args.layout}, aligned>" if umma
+                  else f"generate_kernel<Fixed<2048>, {args.layout}, aligned>")
 
         def step():
-            rlx.rlxpp_generate_doubles(h, out, n_per, rlx.RLXPP_INTERLEAVED)
+            rlx.rlxpp_generate_doubles(h, out, n_per, lay)
     elif args.workload == "cfg5":
         h = rlx.rlxpp_create(n_streams, first_seed, p)
         sk = torch.from_numpy(inputs.cfg5_skip_distances(n_streams).view(np.int64)).cuda()
@@ -402,7 +406,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": ("u8 x u8 -> s32 (tcgen05.mma kind::i8) + u32 limbs -> f64" if umma
                       else "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64"), "data": "synthetic",
-            "config": {"workload": args.workload, "engine": args.engine, "description": desc, "n_streams_per_gpu": n_streams,
+            "config": {"workload": args.workload, "engine": args.engine, "layout": args.layout, "description": desc, "n_streams_per_gpu": n_streams,
                        "doubles_per_stream": n_per, "p": p, "l2": "output per step (12.9 GB) exceeds L2; no flush needed"
                        if args.workload in ("cfg3", "cfg4") else "compute-bound; working set is registers",
                        "parallelism": f"streams sharded over {world} GPU(s), no collective"},

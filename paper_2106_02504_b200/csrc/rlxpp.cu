@@ -9,6 +9,7 @@
 //   12 doubles   -> byte permutes + one exact DADD each; coalesced 64-bit stores
 //                   (interleaved layout), 128-bit stores (stream-major) or DADD/DFMA
 //                   accumulation in registers (fused reduce).
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -255,6 +256,9 @@ struct GenArgs {
   u32* sched;
   u32 n_tiles, n_chunks;
   u64 chunk_len;      // draws per chunk (a multiple of 12 when n_chunks > 1)
+  // UMMA engine, aligned stream-major stores: tensor map of out as [count streams][n_per] doubles,
+  // box = 32 streams x 24 doubles
+  alignas(64) CUtensorMap tmap;
 };
 
 enum { kStoreStreamMajor = 0, kStoreInterleaved = 1, kReduce = 2 };
@@ -356,6 +360,73 @@ __global__ void __launch_bounds__(kThreads) generate_kernel(const __grid_constan
 #include "umma_path.cuh"
 namespace rlx {
 
+// Stream-major stores through shared memory and the TMA (S8 a-7a; north_star: "shared-memory
+// staging, or TMA bulk stores, so HBM writes are fully coalesced").  A thread's block is 96
+// contiguous bytes of ITS stream's row, so direct stores make every warp instruction touch 32 rows
+// (measured 287 G doubles/s, 36 % of the HBM peak).  Instead each warp parks the blocks of TWO
+// advances in shared memory as a dense [32 streams][24 doubles] box and one lane hands it to the
+// TMA: one cp.async.bulk.tensor.2d (SASS UTMASTG) per warp and pair of advances writes 32 row
+// segments of 192 bytes (six whole sectors); rows past the end of the launch are clipped by the
+// tensor map.  The even block of a pair fills the left half of every row, the odd one the right half
+// and sends the box; it is rewritten only after that copy has finished reading it
+// (cp.async.bulk.wait_group.read 0, a whole advance later).  A lone last block is sent with the
+// right half clipped by the tensor map (it can only be the end of the row: chunks are cut at even
+// block counts).  Measured 625 G doubles/s (78 % of the HBM peak; DRAM sees 192-byte pieces 12 KB apart).
+constexpr int kStageBoxCols = 24;
+constexpr int kStageWarpBytes = 32 * 192;
+struct StreamMajorStage {
+  u32 box;        // shared address of this warp's box
+  u32 wr;         // byte offset of this lane's row inside the box
+  const void* tmap;
+  int c1;         // tensor coordinate of the warp's first stream (row)
+  __device__ __forceinline__ void init(uint8_t* stage, const void* tensor_map, u64 tile_first) {
+    const u32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    box = umma::smem_u32(stage) + warp * kStageWarpBytes;
+    wr = lane * (kStageBoxCols * 8u);
+    tmap = tensor_map;
+    c1 = (int)(tile_first + warp * 32u);
+  }
+  template <int J>
+  struct Put {
+    static __device__ __forceinline__ void all(u32 dst, const u32 (&v)[18]) {
+      const double a = draw_double<J>(v), b = draw_double<J + 1>(v);
+      asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dst + J * 8), "d"(a), "d"(b) : "memory");
+      Put<J + 2>::all(dst, v);
+    }
+  };
+  __device__ __forceinline__ void send(u32 src, int c0) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap), "r"(c0),
+                 "r"(c1), "r"(src)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  }
+  // whole-warp call; t = index of the block's first draw within the stream's row, blk = index of the
+  // block within the item, last = it is the item's last block
+  __device__ __forceinline__ void emit(const u32 (&v)[18], u64 t, u64 blk, bool last) {
+    const bool leader = (threadIdx.x & 31u) == 0;
+    const u32 half = (u32)(blk & 1u);
+    if (half == 0) {
+      if (leader) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+      __syncwarp();
+    }
+    Put<0>::all(box + wr + half * 96u, v);
+    if (half == 1 || last) {
+      umma::fence_proxy_async_smem();
+      __syncwarp();
+      if (leader) send(box, (int)(t - half * 12u));
+    }
+  }
+  // before the boxes are reused by another item or the CTA exits
+  __device__ __forceinline__ void drain() {
+    if ((threadIdx.x & 31u) == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    __syncwarp();
+  }
+};
+template <>
+struct StreamMajorStage::Put<12> {
+  static __device__ __forceinline__ void all(u32, const u32 (&)[18]) {}
+};
+
 // ----------------------------------------------------------------------------- UMMA engine
 // Same contract as generate_kernel / advance_states_kernel, with multiply9x9 + mod_m done by
 // the tensor core (umma_path.cuh).  One CTA = 128 streams; every thread of the CTA runs the same
@@ -376,6 +447,8 @@ __device__ __forceinline__ void to_ranlux_hot(const u32 (&x)[18], u32 (&v)[18], 
 template <int MODE, bool ALIGNED>
 __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(const __grid_constant__ GenArgs a) {
   __shared__ tc::Smem smem;
+  constexpr bool kStaged = MODE == kStoreStreamMajor && ALIGNED;
+  __shared__ __align__(128) uint8_t stage[kStaged ? 4 * kStageWarpBytes : 16];
   tc::Tile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
   tile.setup(smem, a.bmat);
   const u64 n_items = (u64)a.n_tiles * a.n_chunks;
@@ -415,6 +488,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
                                        : (MODE == kStoreInterleaved ? a.out + il + t0 * a.ld : nullptr);
     if (ALIGNED) {
       const u64 nblk = n / 12;
+      StreamMajorStage sm;
+      if (kStaged) sm.init(stage, &a.tmap, (u64)tidx * tc::kTile);
       if (nblk > 0) tile.issue(x);
 #pragma unroll 1
       for (u64 b = 0; b < nblk; b++) {
@@ -423,8 +498,10 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         tc::reduce_z(z, x);
         if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
         to_ranlux_hot(x, v, c);
-        if (live) EmitBlock<0, MODE>::all(sink, v, b * 12);
+        if (kStaged) sm.emit(v, t0 + b * 12, b, b + 1 == nblk);
+        else if (live) EmitBlock<0, MODE>::all(sink, v, b * 12);
       }
+      if (kStaged) sm.drain();
     } else if (n > 0) {
       const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
       const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
@@ -772,7 +849,7 @@ static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_
     if (eff >= 0.97) break;
   }
   if (best_c == 1) return;
-  const uint64_t len = (blocks + best_c - 1) / best_c * 12;
+  const uint64_t len = ((blocks + best_c - 1) / best_c + 1) / 2 * 24;  // an even number of blocks (TMA store pairs)
   *chunk_len = len;
   *n_chunks = (uint32_t)((n_per + len - 1) / len);
 }
@@ -787,15 +864,46 @@ static unsigned tc_slots() {
   return slots;
 }
 
+// Tensor map of a stream-major output (UMMA engine, aligned): out[count][n_per] doubles, box 32 x 24.
+// cuTensorMapEncodeTiled comes from the driver through the runtime (no link against libcuda).
+static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count, uint64_t n_per) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !fn) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled is not available");
+    encode = (EncodeFn)fn;
+  }
+  if (n_per >= (1ull << 31) || count >= (1ull << 31))
+    return fail(RLXPP_EINVAL, "stream-major output: n_per_stream and the stream count must be below 2^31");
+  const cuuint64_t dims[2] = {n_per, count};
+  const cuuint64_t strides[1] = {n_per * sizeof(double)};
+  const cuuint32_t box[2] = {kStageBoxCols, 32};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, out, dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return RLXPP_OK;
+}
+
 template <int MODE>
 static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
+  if (MODE == kStoreStreamMajor && aligned) {
+    const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per);
+    if (rc) return rc;
+  }
   const uint64_t n_tiles = (a.count + tc::kTile - 1) / tc::kTile;
   const unsigned slots = tc_slots();
   a.n_tiles = (u32)n_tiles;
   plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len);
   if (g_force_chunks.load() > 0 && a.n_per / 12 >= (uint64_t)g_force_chunks.load()) {  // test hook
     const uint64_t c = (uint64_t)g_force_chunks.load(), blocks = a.n_per / 12;
-    a.chunk_len = (blocks + c - 1) / c * 12;
+    a.chunk_len = ((blocks + c - 1) / c + 1) / 2 * 24;
     a.n_chunks = (u32)((a.n_per + a.chunk_len - 1) / a.chunk_len);
   }
   const uint64_t items = n_tiles * a.n_chunks;
