@@ -200,7 +200,7 @@ def main():
     import numpy as np
     import torch
     import paper_2106_02504_b200 as rlx
-    from paper_2106_02504_b200 import inputs
+    from paper_2106_02504_b200 import inputs, shard
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
@@ -218,7 +218,10 @@ def main():
     umma = args.engine == "umma"
 
     n_streams, n_per, p, desc = WORKLOADS[args.workload]
-    first_seed = 1 + rank * n_streams  # rank g owns seeds 1 + g N .. (g + 1) N
+    # weak scaling: the job has world x n_streams streams, rank g owns the contiguous range g
+    first_stream, my_streams = shard.stream_range(rank, world, world * n_streams)
+    assert my_streams == n_streams
+    first_seed = shard.rank_seed(1, first_stream)
     stream = torch.cuda.current_stream()
 
     # ---------------------------------------------------------------- set up the step
@@ -278,10 +281,7 @@ def main():
     clocks = sampler.stop() if sampler else {}
     total_ms = ev[0].elapsed_time(ev[-1])
     per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
     value = units * world / (ms_per_step * 1e-3)
 
@@ -312,6 +312,16 @@ def main():
                     "frac": alu["frac"], "traffic": None, "peak_source": alu["model"] + f" (DESIGN.md); HBM {peak_src}",
                     "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
     roofline["engine"] = args.engine
+    if umma:
+        # the products as the tensor core sees them: per 128 advances one M128 x N80 x K96 u8 GEMM tile
+        # (2 x 80 x 96 = 15,360 integer ops per advance); int8 dense peak = measured bf16 x 2 (nominal ratio)
+        bf16 = 1647.3
+        if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")):
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                bf16 = json.load(f).get("bf16_tflops", bf16)
+        tops = units / 12.0 * 15360 / (kernel_ms * 1e-3) / 1e12
+        roofline["tensor"] = {"achieved": tops, "peak": 2.0 * bf16, "unit": "TOP/s (u8 x u8 -> s32)", "frac": tops / (2.0 * bf16),
+                              "what": "tcgen05.mma kind::i8 work incl. the K 72->96 and N 72->80 padding; not the binding unit"}
     roofline["doubles_roofline"] = {"alu": roof_alu, "hbm": (None if roof_hbm == float("inf") else roof_hbm),
                                     "min": min(roof_alu, roof_hbm), "frac": doubles_rate / min(roof_alu, roof_hbm),
                                     "what": "north_star's roofline: the slower of nominal IMAD peak / 27 and HBM peak / 8 B"}
@@ -328,7 +338,8 @@ def main():
     traffic_file = os.path.join(ROOT, "profiles", "traffic_r01.json")
     if os.path.exists(traffic_file):
         with open(traffic_file) as f:
-            roofline["traffic"] = json.load(f).get(f"{args.workload}:{args.engine}")
+            key = f"{args.workload}:{args.engine}" + ("" if args.layout == "interleaved" else ":" + args.layout)
+            roofline["traffic"] = json.load(f).get(key)
 
     # ---------------------------------------------------------------- the other engine, same workload (context)
     compare = None
@@ -384,10 +395,7 @@ def main():
             e2e_step()
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = shard.max_over_ranks(dt, dist, "cuda")
         e2e = {"value": units * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": args.e2e_steps,
                "what": "rlxpp_create (seed kernel) + rlxpp_generate_*_host into pinned host memory + rlxpp_destroy, wall clock"}
