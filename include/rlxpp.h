@@ -134,6 +134,24 @@ int rlxpp_get_engine(void);
  * Results never depend on it.  Errors: EINVAL outside [0, 4096]. */
 int rlxpp_set_chunks(int n_chunks);
 
+/* ---- Device-side draw API -------------------------------
+ * include/rlxpp_device.cuh is a header-only per-thread generator for use inside the caller's own
+ * kernels (rlxpp_dev::Stream: load / draw / draw_coop / store).  rlxpp_device_view fills the plain
+ * struct such kernels take (device pointers owned by the handle, valid until rlxpp_destroy); after it
+ * the library assumes nothing about the cursors.  Kernels using the view must be ordered after the
+ * handle's pending work (same CUDA stream, or an event). */
+struct rlxpp_view;
+int rlxpp_device_view(rlxpp_t* h, struct rlxpp_view* out_host);
+/* Ragged generation, written with that device API: stream i draws counts_dev[i] doubles (uint32,
+ * device pointer, n_streams entries).  out_dev[i * ld + t] = draw t of stream i (ld >= max count;
+ * entries beyond a stream's count are left untouched); the _reduce form keeps S = S + d and
+ * Q = fma(d, d, Q) per stream in draw order (sumsq_dev may be NULL).  cooperative != 0 uses the
+ * warp-cooperative advance (draw_coop), 0 the paper's per-thread advance (draw); results are identical.
+ * State and cursors are updated; the draws are the ones rlxpp_generate_doubles would give. */
+int rlxpp_generate_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out_dev, uint64_t ld, int cooperative);
+int rlxpp_generate_ragged_reduce(rlxpp_t* h, const uint32_t* counts_dev, double* sum_dev, double* sumsq_dev,
+                                 int cooperative);
+
 uint64_t rlxpp_n_streams(const rlxpp_t* h);
 /* 1 if the kernels with immediate multipliers serve this luxury level */
 int rlxpp_has_fixed_multiplier(uint32_t p);

@@ -51,6 +51,11 @@ _SIGNATURES = {
     "rlxpp_set_engine": (ctypes.c_int, [ctypes.c_int]),
     "rlxpp_get_engine": (ctypes.c_int, []),
     "rlxpp_set_chunks": (ctypes.c_int, [ctypes.c_int]),
+    "rlxpp_device_view": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "rlxpp_generate_ragged": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64,
+                                             ctypes.c_int]),
+    "rlxpp_generate_ragged_reduce": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                                    ctypes.c_int]),
     "rlxpp_n_streams": (ctypes.c_uint64, [ctypes.c_void_p]),
     "rlxpp_has_fixed_multiplier": (ctypes.c_int, [ctypes.c_uint32]),
     "rlxpp_launch_count": (ctypes.c_uint64, []),
@@ -164,6 +169,27 @@ def rlxpp_generate_doubles(h: Handle, out_dev, n_per_stream: int, layout: int = 
 
 def rlxpp_generate_reduce(h: Handle, sum_dev, sumsq_dev, n_per_stream: int):
     _check(load().rlxpp_generate_reduce(h.ptr, _ptr(sum_dev), _ptr(sumsq_dev), n_per_stream), "rlxpp_generate_reduce")
+
+
+class RlxppView(ctypes.Structure):
+    """rlxpp_view_t of include/rlxpp_device.cuh: what a kernel using the device API takes."""
+    _fields_ = [("st", ctypes.c_void_p), ("n", ctypes.c_uint64), ("A", ctypes.c_void_p)]
+
+
+def rlxpp_device_view(h: Handle) -> RlxppView:
+    v = RlxppView()
+    _check(load().rlxpp_device_view(h.ptr, ctypes.addressof(v)), "rlxpp_device_view")
+    return v
+
+
+def rlxpp_generate_ragged(h: Handle, counts_dev, out_dev, ld: int, cooperative: bool = True):
+    _check(load().rlxpp_generate_ragged(h.ptr, _ptr(counts_dev), _ptr(out_dev), ld, int(cooperative)),
+           "rlxpp_generate_ragged")
+
+
+def rlxpp_generate_ragged_reduce(h: Handle, counts_dev, sum_dev, sumsq_dev, cooperative: bool = True):
+    _check(load().rlxpp_generate_ragged_reduce(h.ptr, _ptr(counts_dev), _ptr(sum_dev), _ptr(sumsq_dev), int(cooperative)),
+           "rlxpp_generate_ragged_reduce")
 
 
 def rlxpp_generate_doubles_host(h: Handle, out_host, n_per_stream: int, layout: int = RLXPP_STREAM_MAJOR):

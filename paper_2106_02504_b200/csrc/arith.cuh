@@ -13,176 +13,22 @@
 #pragma once
 #include <cstdint>
 
+#include "../../include/rlxpp_device.cuh"  // the generic, exact arithmetic (also the public device API)
+
 namespace rlx {
 
-typedef uint32_t u32;
-typedef uint64_t u64;
-typedef int64_t i64;
-
-__host__ __device__ __forceinline__ constexpr u32 m_limb(int j) {
-  return j == 0 ? 1u : (j < 7 ? 0u : (j == 7 ? 0xFFFF0000u : 0xFFFFFFFFu));
-}
-// limbs of 2^240 - 1  (2^576 == 2^240 - 1 mod m)
-__host__ __device__ __forceinline__ constexpr u32 k240_limb(int j) {
-  return j < 7 ? 0xFFFFFFFFu : (j == 7 ? 0x0000FFFFu : 0u);
-}
-
-// ------------------------------------------------------------------ generic product
-// multiply9x9 (sec. 2.1) on 32-bit limbs, column by column: "For every 64 bit in the
-// output, there are up to 9 contributing pairs ... The lower 64 bits of the sum constitutes
-// one entry of the output, while the rest is propagated to the next entry" -- here with
-// 32-bit entries and up to 18 pairs per column (device code multiplies 32-bit values).
-__device__ __forceinline__ void mul18x18(const u32 (&x)[18], const u32 (&y)[18], u32 (&z)[36]) {
-  u64 acc = 0;  // low 64 bits of the running column sum
-  u32 ovf = 0;  // bits 64.. of it
-#pragma unroll
-  for (int k = 0; k < 35; k++) {
-#pragma unroll
-    for (int i = 0; i < 18; i++) {
-      const int j = k - i;
-      if (j >= 0 && j < 18) {
-        const u64 p = (u64)x[i] * y[j];
-        acc += p;
-        ovf += (acc < p);  // P:134-137 Listing 4: branch-free carry
-      }
-    }
-    z[k] = (u32)acc;
-    acc = (acc >> 32) | ((u64)ovf << 32);
-    ovf = 0;
-  }
-  z[35] = (u32)acc;
-}
-
-// x >= m ?
-__device__ __forceinline__ bool ge_m(const u32 (&x)[18]) {
-  u32 all = x[8];
-#pragma unroll
-  for (int j = 9; j < 18; j++) all &= x[j];
-  u32 low = x[0] | x[1] | x[2] | x[3] | x[4] | x[5] | x[6] | (x[7] & 0xFFFFu);
-  return all == 0xFFFFFFFFu && (x[7] >> 16) == 0xFFFFu && low != 0;
-}
-// x -= m for x in [m, 2^576): the top 336 bits are all ones, so x - m = (x mod 2^240) - 1
-__device__ __forceinline__ void sub_m(u32 (&x)[18]) {
-  i64 c = -1;
-#pragma unroll
-  for (int j = 0; j < 8; j++) {
-    const i64 s = (i64)(j == 7 ? (x[7] & 0xFFFFu) : x[j]) + c;
-    x[j] = (u32)s;
-    c = s >> 32;
-  }
-#pragma unroll
-  for (int j = 8; j < 18; j++) x[j] = 0;
-}
-
-// mod_m (sec. 2.2): remainder of a 1152-bit value modulo m "using additions,
-// subtractions, and bit shifts" plus the "fix to ensure that the result is smaller than m
-// in all cases".  Reading c-9:  z = lo + hi 2^576, hi = t1 2^336 + t0, u = t0 + t1,
-//   z == lo - hi - t1 + (u mod 2^336) 2^240 + (u >> 336)(2^240 - 1)   (mod m)
-// summed limb by limb with a signed carry; the final carry k is folded again as
-// k (2^240 - 1), and m is subtracted once if the result is still >= m.
-__device__ __forceinline__ void mod_m36(const u32 (&z)[36], u32 (&r)[18]) {
-  u32 t1[8];
-#pragma unroll
-  for (int j = 0; j < 7; j++) t1[j] = (z[28 + j] >> 16) | (z[29 + j] << 16);
-  t1[7] = z[35] >> 16;
-  u32 u[11];
-  u64 c = 0;
-#pragma unroll
-  for (int j = 0; j < 11; j++) {
-    const u64 s = (u64)(j < 10 ? z[18 + j] : (z[28] & 0xFFFFu)) + (j < 8 ? t1[j] : 0u) + c;
-    u[j] = (u32)s;
-    c = s >> 32;
-  }
-  const u32 ubit = u[10] >> 16;  // u >> 336
-  u[10] &= 0xFFFFu;              // u mod 2^336
-  i64 carry = 0;
-#pragma unroll
-  for (int j = 0; j < 18; j++) {
-    u32 ush = 0;  // limb j of (u mod 2^336) << 240
-    if (j == 7) ush = u[0] << 16;
-    else if (j > 7) ush = (u[j - 7] << 16) | (u[j - 8] >> 16);
-    const i64 s = (i64)z[j] - (i64)z[18 + j] - (i64)(j < 8 ? t1[j] : 0u) + (i64)ush +
-                  (i64)(ubit ? k240_limb(j) : 0u) + carry;
-    r[j] = (u32)s;
-    carry = s >> 32;
-  }
-  // value = r + carry 2^576 == r + carry (2^240 - 1); by the bound in c-9 |carry| <= 1 and one
-  // fold suffices; a second pass (normally with 0) keeps this exact even if it did not.
-#pragma unroll
-  for (int pass = 0; pass < 2; pass++) {
-    const i64 k = carry;
-    carry = 0;
-#pragma unroll
-    for (int j = 0; j < 18; j++) {
-      const i64 s = (i64)r[j] + k * (i64)k240_limb(j) + carry;
-      r[j] = (u32)s;
-      carry = s >> 32;
-    }
-  }
-  if (ge_m(r)) sub_m(r);  // the fix: result < m
-}
-
-// canonical representative of a 640-bit value given as 20 limbs (what the row-reduced
-// product leaves): zero-extend and reduce
-__device__ __forceinline__ void mod_m20(const u32 (&z)[20], u32 (&r)[18]) {
-  u32 zz[36];
-#pragma unroll
-  for (int j = 0; j < 36; j++) zz[j] = j < 20 ? z[j] : 0u;
-  mod_m36(zz, r);
-}
-
-__device__ __forceinline__ void mulmod_generic(const u32 (&x)[18], const u32 (&y)[18], u32 (&r)[18]) {
-  u32 z[36];
-  mul18x18(x, y, z);
-  mod_m36(z, r);
-}
-
-// ------------------------------------------------------------------ LCG -> RANLUX numbers
-// P:39 (sec. 2.3): "converts the LCG state back to RANLUX numbers".  Reading D4 (c-4), exact:
-//   Xh = X >> 336, Xl = X mod 2^336, S = Xl + Xh, D = S 2^240 - S - Xh 2^336 (signed)
-//   T = Xh - [D < 0]   (D >= m is impossible: D <= (2^336 - 1)(2^240 - 1) < m)
-//   V = X + T,  c = (V >> 336) - T
-// X must be canonical (< m).  V = the 24 RANLUX numbers packed, oldest in the low bits.
-__device__ __forceinline__ void to_ranlux_exact(const u32 (&x)[18], u32 (&v)[18], u32& c_out) {
-  u32 xh[8];
-#pragma unroll
-  for (int j = 0; j < 7; j++) xh[j] = (x[10 + j] >> 16) | (x[11 + j] << 16);
-  xh[7] = x[17] >> 16;
-  u32 s[11];  // S = Xl + Xh, up to 337 bits
-  u64 c = 0;
-#pragma unroll
-  for (int j = 0; j < 11; j++) {
-    const u64 t = (u64)(j < 10 ? x[j] : (x[10] & 0xFFFFu)) + (j < 8 ? xh[j] : 0u) + c;
-    s[j] = (u32)t;
-    c = t >> 32;
-  }
-  // sign of D = (S << 240) - S - (Xh << 336), limbs 0..18
-  i64 carry = 0;
-#pragma unroll
-  for (int j = 0; j < 19; j++) {
-    u32 ssh = 0;  // limb j of S << 240
-    if (j == 7) ssh = s[0] << 16;
-    else if (j > 7 && j < 18) ssh = (s[j - 7] << 16) | (s[j - 8] >> 16);
-    else if (j == 18) ssh = s[10] >> 16;
-    u32 xsh = 0;  // limb j of Xh << 336 = the bits of X at and above 336
-    if (j == 10) xsh = x[10] & 0xFFFF0000u;
-    else if (j > 10 && j < 18) xsh = x[j];
-    const i64 t = (i64)ssh - (i64)(j < 11 ? s[j] : 0u) - (i64)xsh + carry;
-    carry = t >> 32;
-  }
-  const u32 neg = carry < 0 ? 1u : 0u;  // D < 0
-  // V = X + Xh - neg
-  i64 cy = -(i64)neg;
-#pragma unroll
-  for (int j = 0; j < 18; j++) {
-    const i64 t = (i64)x[j] + (i64)(j < 8 ? xh[j] : 0u) + cy;
-    v[j] = (u32)t;
-    cy = t >> 32;
-  }
-  // c = (V >> 336) - Xh + neg; (V >> 336) - Xh is 0 or 1, so its low limb decides
-  const u32 vh0 = (v[10] >> 16) | (v[11] << 16);
-  c_out = (vh0 - xh[0]) + neg;
-}
+using rlxpp_dev::detail::u32;
+using rlxpp_dev::detail::u64;
+using rlxpp_dev::detail::i64;
+using rlxpp_dev::detail::m_limb;
+using rlxpp_dev::detail::k240_limb;
+using rlxpp_dev::detail::mul18x18;
+using rlxpp_dev::detail::ge_m;
+using rlxpp_dev::detail::sub_m;
+using rlxpp_dev::detail::mod_m36;
+using rlxpp_dev::detail::mod_m20;
+using rlxpp_dev::detail::mulmod_generic;
+using rlxpp_dev::detail::to_ranlux_exact;
 
 // ------------------------------------------------------------------ hot-path fast forms
 // Row-reduced product: Z = sum_i x_i R_i < 2^613 arrives as E/O accumulators (see

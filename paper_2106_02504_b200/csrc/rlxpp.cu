@@ -666,6 +666,51 @@ __global__ void __launch_bounds__(kThreads) import_kernel(uint4* __restrict__ st
   store_state(st, n, i, x, pos > 12u ? 12u : pos);
 }
 
+// ----------------------------------------------------------------------------- device API (S8 f-1)
+// rlxpp_generate_ragged[_reduce]: every stream draws ITS OWN number of doubles -- the paper's GPU use
+// (one state per thread, threads consume numbers at their own pace).  Written entirely
+// with the public per-thread API of include/rlxpp_device.cuh, of which it is the reference use:
+// COOP = draw_coop() (one advance pass per warp and 12 draws whatever the cursors), else draw()
+// (the paper's per-thread advance, which diverges).
+template <bool COOP, bool REDUCE>
+__global__ void __launch_bounds__(kThreads) ragged_kernel(const rlxpp_view_t view, const u32* __restrict__ counts,
+                                                          double* __restrict__ out, u64 ld, double* __restrict__ sum,
+                                                          double* __restrict__ sumsq) {
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  const bool live = i < view.n;
+  rlxpp_dev::Stream g;
+  if (live) g.load(view, i);
+  const u32 cnt = live ? counts[i] : 0u;
+  double S = 0.0, Q = 0.0;
+  double* row = REDUCE ? nullptr : out + i * ld;
+  if (COOP) {
+    const u32 maxc = __reduce_max_sync(0xFFFFFFFFu, cnt);
+#pragma unroll 1
+    for (u32 t = 0; t < maxc; t++) {
+      const unsigned mask = __ballot_sync(0xFFFFFFFFu, t < cnt);
+      if (t < cnt) {
+        const double d = g.draw_coop(mask);
+        if (REDUCE) { S = S + d; Q = __fma_rn(d, d, Q); }
+        else row[t] = d;
+      }
+    }
+  } else {
+#pragma unroll 1
+    for (u32 t = 0; t < cnt; t++) {
+      const double d = g.draw();
+      if (REDUCE) { S = S + d; Q = __fma_rn(d, d, Q); }
+      else row[t] = d;
+    }
+  }
+  if (live) {
+    g.store(view, i);
+    if (REDUCE) {
+      sum[i] = S;
+      if (sumsq) sumsq[i] = Q;
+    }
+  }
+}
+
 // ----------------------------------------------------------------------------- roofline probes
 // IMAD peak: 8 independent carry chains of IMAD.WIDE.U32.X per thread, nothing else in the loop.
 __global__ void __launch_bounds__(kThreads) imad_peak_kernel(u64* out, u32 iters, u32 seed) {
@@ -1248,6 +1293,45 @@ int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev
   h->uniform_pos = 12;
   h->aligned = h->pos_uniform;
   return RLXPP_OK;
+}
+
+int rlxpp_device_view(rlxpp_t* h, struct rlxpp_view* out_host) {
+  if (!h || !out_host) return fail(RLXPP_EINVAL, "rlxpp_device_view: null argument");
+  out_host->st = h->st;
+  out_host->n = h->n;
+  out_host->A = h->tabA;  // entry 0 of the power table is A itself
+  // kernels of the caller may move the cursors: the library no longer knows them
+  h->pos_uniform = false;
+  h->aligned = false;
+  return RLXPP_OK;
+}
+
+static int launch_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out, uint64_t ld, double* sum, double* sumsq,
+                         int coop, bool reduce) {
+  rlxpp_view_t view;
+  int rc = rlxpp_device_view(h, &view);
+  if (rc) return rc;
+  const unsigned grid = grid_for(h->n);
+  if (reduce) {
+    if (coop) ragged_kernel<true, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else ragged_kernel<false, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+  } else {
+    if (coop) ragged_kernel<true, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else ragged_kernel<false, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+  }
+  LAUNCH_CHECK();
+  return RLXPP_OK;
+}
+
+int rlxpp_generate_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out_dev, uint64_t ld, int cooperative) {
+  if (!h || !counts_dev || !out_dev) return fail(RLXPP_EINVAL, "rlxpp_generate_ragged: null argument");
+  return launch_ragged(h, counts_dev, out_dev, ld, nullptr, nullptr, cooperative, false);
+}
+
+int rlxpp_generate_ragged_reduce(rlxpp_t* h, const uint32_t* counts_dev, double* sum_dev, double* sumsq_dev,
+                                 int cooperative) {
+  if (!h || !counts_dev || !sum_dev) return fail(RLXPP_EINVAL, "rlxpp_generate_ragged_reduce: null argument");
+  return launch_ragged(h, counts_dev, nullptr, 0, sum_dev, sumsq_dev, cooperative, true);
 }
 
 int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream) {

@@ -264,6 +264,68 @@ def test_cfg5_full_size_sampled(rlx, torch, oracle, nthreads):
     assert np.all(sn > 0.4 * per) and np.all(sn < 0.6 * per)  # every stream was reduced
 
 
+# ------------------------------------------------------------------------------------- device API (8f-1)
+@pytest.mark.parametrize("coop", [True, False])
+def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, coop):
+    """include/rlxpp_device.cuh through rlxpp_generate_ragged: every stream draws its own number of
+    doubles (0 .. 70, so lanes of a warp run out of their blocks at different calls), from per-stream
+    cursors, twice in a row, then the library's bulk kernel continues the same streams.  Everything
+    must be the one sequence the oracle gives for that stream; cooperative and per-thread advance agree."""
+    n, p, ld = 1000, 2048, 72
+    dist = inputs.splitmix64(77, n) % np.uint64(30)
+    c1 = (inputs.splitmix64(78, n) % np.uint64(71)).astype(np.uint32)
+    c2 = (inputs.splitmix64(79, n) % np.uint64(71)).astype(np.uint32)
+    c1[:4] = (0, 1, 12, 70)
+    h = rlx.rlxpp_create(n, 3, p)
+    rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    o1 = torch.full((n, ld), -1.0, dtype=torch.float64, device="cuda")
+    o2 = torch.full((n, ld), -1.0, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_ragged(h, torch.from_numpy(c1.view(np.int32)).cuda(), o1, ld, coop)
+    rlx.rlxpp_generate_ragged(h, torch.from_numpy(c2.view(np.int32)).cuda(), o2, ld, coop)
+    tail = 25
+    o3 = torch.empty((n, tail), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, o3, tail, rlx.RLXPP_STREAM_MAJOR)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n, 3), p, 2 * 70 + tail, skips=dist, want=("doubles",), nthreads=nthreads)["doubles"]
+    g1, g2, g3 = o1.cpu().numpy(), o2.cpu().numpy(), o3.cpu().numpy()
+    for i in range(n):
+        a, b = int(c1[i]), int(c2[i])
+        assert_bits_equal(g1[i, :a], ref[i, :a], f"ragged first call, stream {i}")
+        assert_bits_equal(g2[i, :b], ref[i, a:a + b], f"ragged second call, stream {i}")
+        assert_bits_equal(g3[i], ref[i, a + b:a + b + tail], f"bulk kernel after the device API, stream {i}")
+        assert np.all(g1[i, a:] == -1.0) and np.all(g2[i, b:] == -1.0)  # nothing written past a stream's count
+    rlx.rlxpp_destroy(h)
+
+
+@pytest.mark.parametrize("coop", [True, False])
+def test_device_api_ragged_reduce(rlx, torch, oracle, nthreads, coop):
+    n, p = 700, 389
+    cnt = (inputs.splitmix64(5150, n) % np.uint64(200)).astype(np.uint32)
+    h = rlx.rlxpp_create(n, 1, p)
+    rlx.rlxpp_skip(h, 7)
+    s = torch.empty(n, dtype=torch.float64, device="cuda")
+    q = torch.empty(n, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_ragged_reduce(h, torch.from_numpy(cnt.view(np.int32)).cuda(), s, q, coop)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n), p, 7 + 200, want=("doubles",), nthreads=nthreads)["doubles"][:, 7:]
+    S, Q = np.zeros(n), np.zeros(n)
+    from fractions import Fraction
+    for i in range(n):
+        a = b = 0.0
+        for t in range(int(cnt[i])):
+            d = float(ref[i, t])
+            a = a + d
+            b = float(Fraction(d) * Fraction(d) + Fraction(b))  # fma: one correctly rounded result (c-14)
+        S[i], Q[i] = a, b
+    assert_bits_equal(s.cpu().numpy(), S, "ragged sum")
+    assert_bits_equal(q.cpu().numpy(), Q, "ragged sum of squares")
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    for i in (0, 1, 31, 32, 699):
+        Xe, pe, _ = oracle.engine_run(oracle.seed_state(1 + i, p), 12, p, [("skip", 7), ("draw", int(cnt[i]))])
+        assert inputs.limbs_to_int(X[i]) == Xe and int(pos[i]) == pe
+    rlx.rlxpp_destroy(h)
+
+
 # ------------------------------------------------------------------------------------- cursor logic
 def test_unaligned_draw_counts_and_uniform_skip(rlx, torch, oracle, nthreads):
     """Draw counts that are not multiples of 12, interleaved with uniform skips (D8): the
