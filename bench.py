@@ -35,6 +35,8 @@ WORKLOADS = {
     "cfg3": (1 << 20, 1536, 2048, "BASELINE configs[2]: 2^20 streams x 1536 doubles, p=2048, interleaved, 12.9 GB/step"),
     "cfg4": (1 << 18, 6144, 2048, "BASELINE configs[3] at p=2048: 2^18 streams x 6144 doubles, interleaved, 12.9 GB/step"),
     "cfg5": (1 << 18, 49152, 2048, "BASELINE configs[4]: 2^18 streams, random 64-bit skips, 49152 doubles fused to sum/sumsq"),
+    "devapi": (1 << 18, 1200, 2048, "SURVEY 8f-1: device-side draw API (include/rlxpp_device.cuh), 2^18 streams with random "
+                                    "cursors, 1200 draws each summed per stream (rlxpp_generate_ragged_reduce, draw_coop)"),
     "cfg2": ((1 << 20) + 64, 16, 2048, "BASELINE configs[1]: 2^20+64 raw states x 16 advances in place (AoS)"),
 }
 
@@ -215,7 +217,7 @@ def main():
     rlx.load()
     engines = {"umma": rlx.RLXPP_ENGINE_UMMA, "imad": rlx.RLXPP_ENGINE_IMAD}
     rlx.rlxpp_set_engine(engines[args.engine])
-    umma = args.engine == "umma"
+    umma = args.engine == "umma" and args.workload != "devapi"  # the device API advances with IMADs per thread
 
     n_streams, n_per, p, desc = WORKLOADS[args.workload]
     # weak scaling: the job has world x n_streams streams, rank g owns the contiguous range g
@@ -248,6 +250,19 @@ def main():
 
         def step():
             rlx.rlxpp_generate_reduce(h, S, Q, n_per)
+    elif args.workload == "devapi":
+        h = rlx.rlxpp_create(n_streams, first_seed, p)
+        sk = torch.from_numpy(inputs.cfg5_skip_distances(n_streams).view(np.int64)).cuda()
+        rlx.rlxpp_skip_each(h, sk)
+        S = torch.empty(n_streams, dtype=torch.float64, device="cuda")
+        Q = torch.empty(n_streams, dtype=torch.float64, device="cuda")
+        cnt = torch.full((n_streams,), n_per, dtype=torch.int32, device="cuda")
+        units = n_streams * n_per
+        alg_bytes = (2 * 80 + 16 + 4) * n_streams
+        kernel = "ragged_kernel<coop, reduce>"
+
+        def step():
+            rlx.rlxpp_generate_ragged_reduce(h, cnt, S, Q, True)
     else:  # cfg2: raw advances; "doubles" = 12 per advance for the common unit
         h = None
         states = torch.from_numpy(inputs.cfg2_states(1 << 20).view(np.int64)).cuda()
@@ -343,7 +358,7 @@ def main():
 
     # ---------------------------------------------------------------- the other engine, same workload (context)
     compare = None
-    if not args.no_compare:
+    if not args.no_compare and args.workload != "devapi":
         other = "imad" if umma else "umma"
         rlx.rlxpp_set_engine(engines[other])
         step()
@@ -357,6 +372,28 @@ def main():
         compare = {"engine": other, "value": units / (c0.elapsed_time(c1) / 3 * 1e-3), "unit": UNIT, "steps": 3,
                    "n_gpus": 1, "what": "same workload and launch configuration with the other engine, this rank only"}
         rlx.rlxpp_set_engine(engines[args.engine])
+
+    devapi = None
+    if args.workload == "devapi":
+        def timed(fn, reps=3):
+            fn()
+            torch.cuda.synchronize()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record(stream)
+            for _ in range(reps):
+                fn()
+            c1.record(stream)
+            torch.cuda.synchronize()
+            return units / (c0.elapsed_time(c1) / reps * 1e-3)
+        per_thread = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h, cnt, S, Q, False))
+        h2 = rlx.rlxpp_create(n_streams, first_seed, p)  # fresh handle: every cursor 12 (the paper's aligned case)
+        aligned_pt = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h2, cnt, S, Q, False))
+        aligned_coop = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h2, cnt, S, Q, True))
+        rlx.rlxpp_destroy(h2)
+        devapi = {"unit": UNIT, "random_cursors_draw_coop": None, "random_cursors_draw": per_thread,
+                  "aligned_cursors_draw": aligned_pt, "aligned_cursors_draw_coop": aligned_coop,
+                  "what": "PAPER.md lines 174-176: per-thread skipping made the paper's GPU run 7x slower; draw_coop "
+                          "keeps one advance pass per warp and 12 draws whatever the cursors"}
 
     # ---------------------------------------------------------------- end to end (host buffers)
     e2e = None
@@ -422,6 +459,9 @@ def main():
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "other_engine": compare,
         }
+        if devapi is not None:
+            devapi["random_cursors_draw_coop"] = value
+            line["device_api"] = devapi
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
