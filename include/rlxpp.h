@@ -134,6 +134,27 @@ int rlxpp_get_engine(void);
  * Results never depend on it.  Errors: EINVAL outside [0, 4096]. */
 int rlxpp_set_chunks(int n_chunks);
 
+/* ---- Other output forms of the same draws ("IntRndm") --------------
+ * rlxpp_generate_u48: the 48-bit integers k themselves (the double is k 2^-48), one uint64_t each.
+ * rlxpp_generate_floats: the 24-bit RANLUX numbers as floats x 2^-24 in [0, 1), exact; one 48-bit draw
+ *   gives two floats, low number (the older one) first, so n_per_stream must be even and the cursor
+ *   moves by n_per_stream / 2 draws.
+ * Layouts as rlxpp_generate_doubles, in elements of the output type (INTERLEAVED floats:
+ * out[k * n_streams + i], k = float index).  Same cursor, same sequence: calls of all generate
+ * functions interleave freely.  Both always run on the UMMA engine's kernels.  Errors as
+ * rlxpp_generate_doubles, plus EINVAL for an odd float count. */
+int rlxpp_generate_u48(rlxpp_t* h, uint64_t* out_dev, uint64_t n_per_stream, int layout);
+int rlxpp_generate_floats(rlxpp_t* h, float* out_dev, uint64_t n_per_stream, int layout);
+
+/* ---- Host engine ------------------------------------------
+ * ONE stream continued on the host, with the library's own host arithmetic: the same sequence as the
+ * device kernels, so a stream can move between host and device mid-stream through rlxpp_get_state /
+ * rlxpp_set_state.  lcg_inout: 9 uint64_t (LCG form, any value < 2^576, canonical on return);
+ * pos_inout: cursor 0..12; first `skip` draws are skipped (any 64-bit count), then `n` doubles are
+ * written to out_host.  Needs no device.  Errors: EINVAL (null pointer, p == 0, cursor > 12). */
+int rlxpp_host_generate(uint64_t* lcg_inout, uint32_t* pos_inout, uint32_t p, uint64_t skip, uint64_t n,
+                        double* out_host);
+
 /* ---- Device-side draw API -------------------------------
  * include/rlxpp_device.cuh is a header-only per-thread generator for use inside the caller's own
  * kernels (rlxpp_dev::Stream: load / draw / draw_coop / store).  rlxpp_device_view fills the plain

@@ -51,6 +51,10 @@ _SIGNATURES = {
     "rlxpp_set_engine": (ctypes.c_int, [ctypes.c_int]),
     "rlxpp_get_engine": (ctypes.c_int, []),
     "rlxpp_set_chunks": (ctypes.c_int, [ctypes.c_int]),
+    "rlxpp_generate_u48": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
+    "rlxpp_generate_floats": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
+    "rlxpp_host_generate": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64,
+                                           ctypes.c_uint64, ctypes.c_void_p]),
     "rlxpp_device_view": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
     "rlxpp_generate_ragged": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64,
                                              ctypes.c_int]),
@@ -169,6 +173,24 @@ def rlxpp_generate_doubles(h: Handle, out_dev, n_per_stream: int, layout: int = 
 
 def rlxpp_generate_reduce(h: Handle, sum_dev, sumsq_dev, n_per_stream: int):
     _check(load().rlxpp_generate_reduce(h.ptr, _ptr(sum_dev), _ptr(sumsq_dev), n_per_stream), "rlxpp_generate_reduce")
+
+
+def rlxpp_generate_u48(h: Handle, out_dev, n_per_stream: int, layout: int = RLXPP_STREAM_MAJOR):
+    _check(load().rlxpp_generate_u48(h.ptr, _ptr(out_dev), n_per_stream, layout), "rlxpp_generate_u48")
+
+
+def rlxpp_generate_floats(h: Handle, out_dev, n_per_stream: int, layout: int = RLXPP_STREAM_MAJOR):
+    _check(load().rlxpp_generate_floats(h.ptr, _ptr(out_dev), n_per_stream, layout), "rlxpp_generate_floats")
+
+
+def rlxpp_host_generate(lcg: np.ndarray, pos: int, p: int, skip: int, n: int):
+    """-> (doubles[n], new lcg uint64[9], new cursor); host only."""
+    state = np.ascontiguousarray(lcg, dtype=np.uint64).copy()
+    cur = ctypes.c_uint32(pos)
+    out = np.empty(max(n, 1), np.float64)
+    _check(load().rlxpp_host_generate(state.ctypes.data, ctypes.addressof(cur), p, skip & (2**64 - 1), n, out.ctypes.data),
+           "rlxpp_host_generate")
+    return out[:n], state, int(cur.value)
 
 
 class RlxppView(ctypes.Structure):

@@ -157,5 +157,31 @@ inline Big pow2k(Big base, int k) {  // base^(2^k)
   return base;
 }
 
+// LCG state -> the 24 RANLUX numbers packed in 576 bits + carry (reading D4, shift/add form):
+//   Xh = X >> 336, S = (X mod 2^336) + Xh, D = S 2^240 - S - Xh 2^336, T = Xh - [D < 0], V = X + T,
+//   c = (V >> 336) - T.  X must be canonical (< m).
+inline void to_ranlux(const Big& X, uint32_t v[18], uint32_t* carry) {
+  const Big Xh = Big::shr(X, 336);
+  const Big S = Big::add(Big::low_bits(X, 336), Xh);
+  const bool neg = Big::cmp(Big::shl(S, 240), Big::add(S, Big::shl(Xh, 336))) < 0;
+  const Big T = neg ? Big::sub(Xh, Big(1)) : Xh;  // D < 0 implies Xh >= 1
+  const Big V = Big::add(X, T);
+  V.to_u32x18(v);
+  if (carry) {
+    const Big d = Big::sub(Big::shr(V, 336), T);
+    *carry = d.is_zero() ? 0u : d.w[0];
+  }
+}
+inline Big from_u64x9(const uint64_t in[9]) {
+  Big r;
+  r.w.resize(18);
+  for (int i = 0; i < 9; i++) {
+    r.w[2 * i] = (uint32_t)in[i];
+    r.w[2 * i + 1] = (uint32_t)(in[i] >> 32);
+  }
+  r.trim();
+  return r;
+}
+
 }  // namespace host
 }  // namespace rlx

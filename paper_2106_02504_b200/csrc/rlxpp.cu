@@ -262,49 +262,74 @@ struct GenArgs {
 };
 
 enum { kStoreStreamMajor = 0, kStoreInterleaved = 1, kReduce = 2 };
+// What a 48-bit draw is written as (S8 f-2): the double k 2^-48; the integer k as uint64; or its two
+// 24-bit RANLUX numbers as floats x 2^-24 (low number first).  Every form is 8 bytes per draw, carried
+// through the emission code as the bit pattern of a double.
+enum { kF64 = 0, kU48 = 1, kF32 = 2 };
 
-template <int MODE>
+template <int OUT, int J>
+__device__ __forceinline__ double draw_value(const u32 (&v)[18]) {
+  if (OUT == kF64) return draw_double<J>(v);
+  u32 lo, hi;  // bits 0..31 and 32..47 of the draw
+  if (J % 2 == 0) {
+    lo = v[3 * J / 2];
+    hi = v[3 * J / 2 + 1] & 0xFFFFu;
+  } else {
+    lo = __byte_perm(v[(3 * J - 1) / 2], v[(3 * J + 1) / 2], 0x5432);
+    hi = v[(3 * J + 1) / 2] >> 16;
+  }
+  if (OUT == kU48) return __hiloint2double((int)hi, (int)lo);
+  const float f0 = __uint2float_rn(lo & 0xFFFFFFu) * 0x1p-24f;               // RANLUX number 2J (exact)
+  const float f1 = __uint2float_rn(__byte_perm(lo, hi, 0x6543)) * 0x1p-24f;  // number 2J + 1 = bits 24..47
+  return __hiloint2double(__float_as_int(f1), __float_as_int(f0));
+}
+
+template <int MODE, int OUT = kF64>
 struct Sink {
-  double* p;      // STREAM_MAJOR: &out[i_local * n_per]; INTERLEAVED: &out[i_local]
+  double* p;      // STREAM_MAJOR: &out[i_local * n_per]; INTERLEAVED: &out[i_local] (kF32: float index i_local)
   u64 ld;
   double S, Q;
   __device__ __forceinline__ void emit(u64 t, double d) {
     if (MODE == kStoreStreamMajor) p[t] = d;
-    else if (MODE == kStoreInterleaved) __stcs(p + t * ld, d);
+    else if (MODE == kStoreInterleaved && OUT == kF32) {  // floats 2t and 2t + 1 of the stream: rows of 4-byte elements
+      float* pf = reinterpret_cast<float*>(p);
+      __stcs(pf + (2 * t) * ld, __int_as_float(__double2loint(d)));
+      __stcs(pf + (2 * t + 1) * ld, __int_as_float(__double2hiint(d)));
+    } else if (MODE == kStoreInterleaved) __stcs(p + t * ld, d);
     else { S = S + d; Q = __fma_rn(d, d, Q); }
   }
 };
 
-template <int J, int MODE>
+template <int J, int MODE, int OUT = kF64>
 struct EmitBlock {
   // all 12 draws of block v go to output indices t0 .. t0 + 11 (VEC: t0 is even and p is 16-byte aligned)
   template <bool VEC = true>
-  static __device__ __forceinline__ void all(Sink<MODE>& s, const u32 (&v)[18], u64 t0) {
+  static __device__ __forceinline__ void all(Sink<MODE, OUT>& s, const u32 (&v)[18], u64 t0) {
     if (MODE == kStoreStreamMajor && VEC) {
       if (J % 2 == 0) {  // two draws per 128-bit store (p + t0 is 16-byte aligned: n_per % 12 == 0)
-        double2 d2 = make_double2(draw_double<J>(v), draw_double<J + 1>(v));
+        double2 d2 = make_double2(draw_value<OUT, J>(v), draw_value<OUT, J + 1>(v));
         __stcs(reinterpret_cast<double2*>(s.p + t0 + J), d2);
       }
     } else {
-      s.emit(t0 + J, draw_double<J>(v));
+      s.emit(t0 + J, draw_value<OUT, J>(v));
     }
-    EmitBlock<J + 1, MODE>::template all<VEC>(s, v, t0);
+    EmitBlock<J + 1, MODE, OUT>::template all<VEC>(s, v, t0);
   }
   // draw J of the block at absolute draw position q0 + J is output index q0 + J - pos if in [0, n)
-  static __device__ __forceinline__ void masked(Sink<MODE>& s, const u32 (&v)[18], u64 q0, u32 pos, u64 n) {
+  static __device__ __forceinline__ void masked(Sink<MODE, OUT>& s, const u32 (&v)[18], u64 q0, u32 pos, u64 n) {
     const u64 t = q0 + J - pos;  // wraps when q0 + J < pos: then t >= n
     const bool valid = t < n;
-    const double d = draw_double<J>(v);
+    const double d = draw_value<OUT, J>(v);
     if (MODE == kReduce) s.emit(t, valid ? d : 0.0);  // + 0.0 and fma(0, 0, Q) are exact no-ops
     else if (valid) s.emit(t, d);
-    EmitBlock<J + 1, MODE>::masked(s, v, q0, pos, n);
+    EmitBlock<J + 1, MODE, OUT>::masked(s, v, q0, pos, n);
   }
 };
-template <int MODE>
-struct EmitBlock<12, MODE> {
+template <int MODE, int OUT>
+struct EmitBlock<12, MODE, OUT> {
   template <bool VEC = true>
-  static __device__ __forceinline__ void all(Sink<MODE>&, const u32 (&)[18], u64) {}
-  static __device__ __forceinline__ void masked(Sink<MODE>&, const u32 (&)[18], u64, u32, u64) {}
+  static __device__ __forceinline__ void all(Sink<MODE, OUT>&, const u32 (&)[18], u64) {}
+  static __device__ __forceinline__ void masked(Sink<MODE, OUT>&, const u32 (&)[18], u64, u32, u64) {}
 };
 
 // ALIGNED: every cursor is 12 and n_per % 12 == 0: n_per / 12 advances, no masks.
@@ -386,12 +411,12 @@ struct StreamMajorStage {
     tmap = tensor_map;
     c1 = (int)(tile_first + warp * 32u);
   }
-  template <int J>
+  template <int OUT, int J>
   struct Put {
     static __device__ __forceinline__ void all(u32 dst, const u32 (&v)[18]) {
-      const double a = draw_double<J>(v), b = draw_double<J + 1>(v);
+      const double a = draw_value<OUT, J>(v), b = draw_value<OUT, J + 1>(v);
       asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dst + J * 8), "d"(a), "d"(b) : "memory");
-      Put<J + 2>::all(dst, v);
+      Put<OUT, J + 2>::all(dst, v);
     }
   };
   __device__ __forceinline__ void send(u32 src, int c0) {
@@ -402,6 +427,7 @@ struct StreamMajorStage {
   }
   // whole-warp call; t = index of the block's first draw within the stream's row, blk = index of the
   // block within the item, last = it is the item's last block
+  template <int OUT>
   __device__ __forceinline__ void emit(const u32 (&v)[18], u64 t, u64 blk, bool last) {
     const bool leader = (threadIdx.x & 31u) == 0;
     const u32 half = (u32)(blk & 1u);
@@ -409,7 +435,7 @@ struct StreamMajorStage {
       if (leader) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
       __syncwarp();
     }
-    Put<0>::all(box + wr + half * 96u, v);
+    Put<OUT, 0>::all(box + wr + half * 96u, v);
     if (half == 1 || last) {
       umma::fence_proxy_async_smem();
       __syncwarp();
@@ -422,8 +448,8 @@ struct StreamMajorStage {
     __syncwarp();
   }
 };
-template <>
-struct StreamMajorStage::Put<12> {
+template <int OUT>
+struct StreamMajorStage::Put<OUT, 12> {
   static __device__ __forceinline__ void all(u32, const u32 (&)[18]) {}
 };
 
@@ -444,7 +470,7 @@ __device__ __forceinline__ void to_ranlux_hot(const u32 (&x)[18], u32 (&v)[18], 
 // partial wave shrinks from a whole tile's work to one chunk's (cfg4 / cfg5: 2,048 tiles over
 // 148 x 5 CTAs).  A CTA that waits for chunk c - 1 of its tile waits for an EARLIER ticket, which a
 // resident CTA holds: no deadlock whatever the number of resident CTAs.
-template <int MODE, bool ALIGNED>
+template <int MODE, bool ALIGNED, int OUT = kF64>
 __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(const __grid_constant__ GenArgs a) {
   __shared__ tc::Smem smem;
   constexpr bool kStaged = MODE == kStoreStreamMajor && ALIGNED;
@@ -476,7 +502,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
 #pragma unroll
     for (int j = 0; j < 18; j++) x[j] = 0;
     if (live) load_state(a.st, a.n_total, i, x, pos);
-    Sink<MODE> sink;
+    Sink<MODE, OUT> sink;
     sink.ld = a.ld;
     sink.S = 0.0;
     sink.Q = 0.0;
@@ -484,8 +510,11 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
       sink.S = __ldcg(a.sum + il);
       sink.Q = __ldcg(a.sumsq + il);
     }
-    sink.p = MODE == kStoreStreamMajor ? a.out + il * a.n_per + t0
-                                       : (MODE == kStoreInterleaved ? a.out + il + t0 * a.ld : nullptr);
+    if (MODE == kStoreStreamMajor) sink.p = a.out + il * a.n_per + t0;
+    else if (MODE == kStoreInterleaved && OUT == kF32)  // 4-byte elements: float il of float row 2 t0
+      sink.p = reinterpret_cast<double*>(reinterpret_cast<float*>(a.out) + il + 2 * t0 * a.ld);
+    else if (MODE == kStoreInterleaved) sink.p = a.out + il + t0 * a.ld;
+    else sink.p = nullptr;
     if (ALIGNED) {
       const u64 nblk = n / 12;
       StreamMajorStage sm;
@@ -498,8 +527,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         tc::reduce_z(z, x);
         if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
         to_ranlux_hot(x, v, c);
-        if (kStaged) sm.emit(v, t0 + b * 12, b, b + 1 == nblk);
-        else if (live) EmitBlock<0, MODE>::all(sink, v, b * 12);
+        if (kStaged) sm.emit<OUT>(v, t0 + b * 12, b, b + 1 == nblk);
+        else if (live) EmitBlock<0, MODE, OUT>::all(sink, v, b * 12);
       }
       if (kStaged) sm.drain();
     } else if (n > 0) {
@@ -507,7 +536,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
       const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
       if (pos < 12) {
         to_ranlux_exact(x, v, c);
-        if (live) EmitBlock<0, MODE>::masked(sink, v, 0, pos, n);
+        if (live) EmitBlock<0, MODE, OUT>::masked(sink, v, 0, pos, n);
       }
       tile.issue(x);
       // blocks 1 .. smax - 2 lie wholly inside [0, n) for every cursor (last >= smax - 1): no masks
@@ -519,7 +548,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         tc::reduce_z(z, x);
         tile.issue(x);
         to_ranlux_hot(x, v, c);
-        if (live) EmitBlock<0, MODE>::template all<false>(sink, v, s * 12 - pos);
+        if (live) EmitBlock<0, MODE, OUT>::template all<false>(sink, v, s * 12 - pos);
       }
 #pragma unroll 1
       for (; s <= smax; s++) {
@@ -534,7 +563,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         if (s < smax) tile.issue(x);
         if (take) {
           to_ranlux_hot(x, v, c);
-          if (live) EmitBlock<0, MODE>::masked(sink, v, s * 12, pos, n);
+          if (live) EmitBlock<0, MODE, OUT>::masked(sink, v, s * 12, pos, n);
         }
       }
       pos = (u32)((u64)pos + n - 12 * last);
@@ -936,7 +965,7 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
   return RLXPP_OK;
 }
 
-template <int MODE>
+template <int MODE, int OUT = kF64>
 static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   if (MODE == kStoreStreamMajor && aligned) {
     const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per);
@@ -954,8 +983,8 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   const uint64_t items = n_tiles * a.n_chunks;
   const unsigned grid = (unsigned)(items < slots ? items : slots);
   CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
-  if (aligned) tc_generate_kernel<MODE, true><<<grid, tc::kTile, 0, s>>>(a);
-  else tc_generate_kernel<MODE, false><<<grid, tc::kTile, 0, s>>>(a);
+  if (aligned) tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, 0, s>>>(a);
+  else tc_generate_kernel<MODE, false, OUT><<<grid, tc::kTile, 0, s>>>(a);
   LAUNCH_CHECK();
   return RLXPP_OK;
 }
@@ -1202,6 +1231,38 @@ int rlxpp_generate_reduce(rlxpp_t* h, double* sum_dev, double* sumsq_dev, uint64
   return RLXPP_OK;
 }
 
+// 48-bit integers and 24-bit floats (S8 f-2): always the UMMA engine's kernels.
+static int generate_other(rlxpp_t* h, void* out_dev, uint64_t n_draws, int layout, int kind, const char* who) {
+  if (!h) return fail(RLXPP_EINVAL, "%s: null handle", who);
+  if (layout != RLXPP_STREAM_MAJOR && layout != RLXPP_INTERLEAVED) return fail(RLXPP_EINVAL, "%s: unknown layout %d", who, layout);
+  if (n_draws == 0) return RLXPP_OK;
+  if (!out_dev) return fail(RLXPP_EINVAL, "%s: null output", who);
+  if ((uintptr_t)out_dev % 16) return fail(RLXPP_EINVAL, "%s: output must be 16-byte aligned", who);
+  GenArgs a;
+  a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = (double*)out_dev; a.ld = h->n;
+  a.n_per = n_draws; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
+  const bool aligned = h->aligned && n_draws % 12 == 0;
+  int rc;
+  if (kind == kU48)
+    rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor, kU48>(a, aligned, h->stream)
+                                      : launch_tc_generate_mode<kStoreInterleaved, kU48>(a, aligned, h->stream);
+  else
+    rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor, kF32>(a, aligned, h->stream)
+                                      : launch_tc_generate_mode<kStoreInterleaved, kF32>(a, aligned, h->stream);
+  if (rc) return rc;
+  after_generate(h, n_draws);
+  return RLXPP_OK;
+}
+
+int rlxpp_generate_u48(rlxpp_t* h, uint64_t* out_dev, uint64_t n_per_stream, int layout) {
+  return generate_other(h, out_dev, n_per_stream, layout, kU48, "rlxpp_generate_u48");
+}
+
+int rlxpp_generate_floats(rlxpp_t* h, float* out_dev, uint64_t n_per_stream, int layout) {
+  if (n_per_stream % 2) return fail(RLXPP_EINVAL, "rlxpp_generate_floats: n_per_stream must be even (two floats per 48-bit draw)");
+  return generate_other(h, out_dev, n_per_stream / 2, layout, kF32, "rlxpp_generate_floats");
+}
+
 static int ensure_staging(rlxpp_t* h, size_t bytes_each) {
   if (!h->copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
   for (int b = 0; b < 2; b++) {
@@ -1292,6 +1353,46 @@ int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev
   h->pos_uniform = pos_dev == nullptr;
   h->uniform_pos = 12;
   h->aligned = h->pos_uniform;
+  return RLXPP_OK;
+}
+
+// ---- host engine (S8 f-3; the same sequence on the host, so that control can move
+// between host and device mid-stream).  Plain host code on csrc/host_bigint.h; no device needed.
+int rlxpp_host_generate(uint64_t* lcg_inout, uint32_t* pos_inout, uint32_t p, uint64_t skip, uint64_t n,
+                        double* out_host) {
+  if (!lcg_inout || !pos_inout || p == 0 || (n > 0 && !out_host))
+    return fail(RLXPP_EINVAL, "rlxpp_host_generate: null argument or p == 0");
+  if (*pos_inout > 12) return fail(RLXPP_EINVAL, "rlxpp_host_generate: cursor %u > 12", *pos_inout);
+  const host::Big A = host::multiplier_ap(p);
+  host::Big X = host::reduce(host::from_u64x9(lcg_inout));
+  uint32_t pos = *pos_inout;
+  if (skip > 0) {  // D8: k = floor((pos + skip - 1) / 12) without 64-bit overflow
+    const uint64_t t = skip - 1;
+    const uint32_t total = (uint32_t)(t % 12) + pos;
+    const uint64_t k = t / 12 + total / 12;
+    X = host::mulmod(host::powmod(A, k), X);
+    pos = total % 12 + 1;
+  }
+  uint32_t v[18];
+  bool have_block = false;
+  for (uint64_t t = 0; t < n; t++) {
+    if (pos == 12) {
+      X = host::mulmod(A, X);
+      pos = 0;
+      have_block = false;
+    }
+    if (!have_block) {
+      host::to_ranlux(X, v, nullptr);
+      have_block = true;
+    }
+    const uint32_t w = (3 * pos) >> 1;
+    const uint64_t k = (pos & 1) ? ((uint64_t)v[w] >> 16) | ((uint64_t)v[w + 1] << 16)
+                                 : (uint64_t)v[w] | ((uint64_t)(v[w + 1] & 0xFFFFu) << 32);
+    out_host[t] = (double)(int64_t)k * 0x1p-48;
+    pos++;
+  }
+  X.to_u64x9(lcg_inout);
+  *pos_inout = pos;
   return RLXPP_OK;
 }
 

@@ -264,6 +264,69 @@ def test_cfg5_full_size_sampled(rlx, torch, oracle, nthreads):
     assert np.all(sn > 0.4 * per) and np.all(sn < 0.6 * per)  # every stream was reduced
 
 
+# ------------------------------------------------------------------------------------- other outputs (8f-2)
+def _floats_of(ints):
+    """The two 24-bit RANLUX numbers of every 48-bit draw as floats x 2^-24 (exact), low number first."""
+    lo = (ints & np.uint64(0xFFFFFF)).astype(np.float32) * np.float32(2.0**-24)
+    hi = (ints >> np.uint64(24)).astype(np.float32) * np.float32(2.0**-24)
+    return np.stack([lo, hi], axis=-1).reshape(ints.shape[0], -1)
+
+
+@pytest.mark.parametrize("aligned", [True, False])
+def test_u48_and_float_outputs_are_the_same_draws(rlx, torch, oracle, nthreads, aligned):
+    """rlxpp_generate_u48 / rlxpp_generate_floats give the 48-bit integers and the 24-bit numbers of the
+    SAME sequence as the doubles, in both layouts, interleaved with double draws on one cursor."""
+    n, p = 700, 2048
+    nd = 48 if aligned else 41          # draws per call
+    h = rlx.rlxpp_create(n, 8, p)
+    dist = None
+    if not aligned:
+        dist = inputs.splitmix64(31337, n) % np.uint64(50)
+        rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    u_sm = torch.zeros((n, nd), dtype=torch.int64, device="cuda")
+    rlx.rlxpp_generate_u48(h, u_sm, nd, rlx.RLXPP_STREAM_MAJOR)
+    u_il = torch.zeros((nd, n), dtype=torch.int64, device="cuda")
+    rlx.rlxpp_generate_u48(h, u_il, nd, rlx.RLXPP_INTERLEAVED)
+    f_sm = torch.zeros((n, 2 * nd), dtype=torch.float32, device="cuda")
+    rlx.rlxpp_generate_floats(h, f_sm, 2 * nd, rlx.RLXPP_STREAM_MAJOR)
+    f_il = torch.zeros((2 * nd, n), dtype=torch.float32, device="cuda")
+    rlx.rlxpp_generate_floats(h, f_il, 2 * nd, rlx.RLXPP_INTERLEAVED)
+    d = torch.zeros((n, nd), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, d, nd, rlx.RLXPP_STREAM_MAJOR)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n, 8), p, 5 * nd, skips=dist, want=("ints", "doubles", "state"), nthreads=nthreads)
+    ints = ref["ints"]
+    assert np.array_equal(u_sm.cpu().numpy().view(np.uint64), ints[:, :nd])
+    assert np.array_equal(u_il.cpu().numpy().view(np.uint64).T, ints[:, nd:2 * nd])
+    assert np.array_equal(f_sm.cpu().numpy().view(np.uint32), _floats_of(ints[:, 2 * nd:3 * nd]).view(np.uint32))
+    assert np.array_equal(f_il.cpu().numpy().T.copy().view(np.uint32), _floats_of(ints[:, 3 * nd:4 * nd]).view(np.uint32))
+    assert_bits_equal(d.cpu().numpy(), ref["doubles"][:, 4 * nd:], "doubles after the other output forms")
+    check_state(rlx, torch, h, ref, "after u48 / floats")
+    fl = f_sm.cpu().numpy()
+    assert fl.min() >= 0.0 and fl.max() < 1.0 and np.all(fl * 2.0**24 == np.floor(fl * 2.0**24))  # 2^-24 lattice
+    with pytest.raises(rlx.RlxppError, match="even"):
+        rlx.rlxpp_generate_floats(h, f_sm, 7, rlx.RLXPP_STREAM_MAJOR)
+    rlx.rlxpp_destroy(h)
+
+
+def test_p24_floats_are_the_raw_ranlux_numbers(rlx, torch, oracle):
+    """p = 24: the floats are the subtract-with-borrow numbers themselves (x 2^-24), one by one, from
+    the oracle's direct SWB stepper (reading c-13)."""
+    n, per = 40, 240
+    h = rlx.rlxpp_create(n, 1, 24)
+    out = torch.empty((n, per), dtype=torch.float32, device="cuda")
+    rlx.rlxpp_generate_floats(h, out, per, rlx.RLXPP_STREAM_MAJOR)
+    got = (out.cpu().numpy().astype(np.float64) * 2.0**24).astype(np.uint64)
+    for i in (0, 7, 39):
+        V, c = oracle.to_ranlux(oracle.seed_state(1 + i, 24))
+        want = []
+        for _ in range(per // 24):
+            V, c = oracle.swb_steps(V, c, 24)
+            want += [(V >> (24 * j)) & (2**24 - 1) for j in range(24)]
+        assert [int(v) for v in got[i]] == want
+    rlx.rlxpp_destroy(h)
+
+
 # ------------------------------------------------------------------------------------- device API (8f-1)
 @pytest.mark.parametrize("coop", [True, False])
 def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, coop):
@@ -323,6 +386,29 @@ def test_device_api_ragged_reduce(rlx, torch, oracle, nthreads, coop):
     for i in (0, 1, 31, 32, 699):
         Xe, pe, _ = oracle.engine_run(oracle.seed_state(1 + i, p), 12, p, [("skip", 7), ("draw", int(cnt[i]))])
         assert inputs.limbs_to_int(X[i]) == Xe and int(pos[i]) == pe
+    rlx.rlxpp_destroy(h)
+
+
+def test_host_engine_hands_over_with_the_device(rlx, torch, oracle):
+    """a stream moves device -> host -> device mid-block and
+    stays one sequence: get_state, rlxpp_host_generate on the host, set_state, generate on the device."""
+    n, p = 130, 2048
+    h = rlx.rlxpp_create(n, 21, p)
+    a = torch.empty((n, 17), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, a, 17, rlx.RLXPP_STREAM_MAJOR)  # cursor 5 in the second block
+    V, c, pos, X = gpu_state(rlx, torch, h)
+    host_draws = np.empty((n, 20))
+    Xn, posn = X.copy(), pos.copy()
+    for i in range(n):
+        host_draws[i], Xn[i], posn[i] = rlx.rlxpp_host_generate(X[i], int(pos[i]), p, 3, 20)  # skip 3, draw 20
+    rlx.rlxpp_set_state(h, torch.from_numpy(Xn.view(np.int64)).cuda(), torch.from_numpy(posn.astype(np.int32)).cuda())
+    b = torch.empty((n, 30), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, b, 30, rlx.RLXPP_STREAM_MAJOR)
+    torch.cuda.synchronize()
+    ref = oracle.streams(inputs.seeds(n, 21), p, 17 + 3 + 20 + 30, want=("doubles",))["doubles"]
+    assert_bits_equal(a.cpu().numpy(), ref[:, :17], "device part 1")
+    assert_bits_equal(host_draws, ref[:, 20:40], "host part")
+    assert_bits_equal(b.cpu().numpy(), ref[:, 40:], "device part 2")
     rlx.rlxpp_destroy(h)
 
 

@@ -78,3 +78,46 @@ def test_engine_selection_and_errors_without_gpu():
     if not torch.cuda.is_available():  # no CPU fallback: creation must fail, not compute on the host
         with pytest.raises(rlx.RlxppError):
             rlx.rlxpp_create(16, 1, 2048, cuda_stream=0)
+
+
+# ---------------------------------------------------------------- host engine
+def _py_stream(X, pos, A, n):
+    """Python big-integer model of D4 / D6 / D8, written here (closed form V = floor(2^576 X / m))."""
+    out = []
+    for _ in range(n):
+        if pos == 12:
+            X, pos = A * X % M, 0
+        V = (X << 576) // M
+        out.append((V >> (48 * pos)) & ((1 << 48) - 1))
+        pos += 1
+    return out, X, pos
+
+
+def _limbs(x):
+    return np.array([(x >> (64 * i)) & (2**64 - 1) for i in range(9)], dtype=np.uint64)
+
+
+@pytest.mark.parametrize("p", [2048, 24, 389])
+def test_host_engine_matches_big_integer_model(p):
+    A = pow(A1, p, M)
+    X0 = pow(A, (1 << 96) * 1, M)  # seed 1 (reading c-7)
+    d, st, pos = rlx.rlxpp_host_generate(_limbs(X0), 12, p, 0, 40)
+    want, Xe, pe = _py_stream(X0, 12, A, 40)
+    assert [int(v * 2.0**48) for v in d] == want and to_int(st) == Xe and pos == pe
+    if p == 2048:  # survey vectors (SURVEY 8c): first three draws of seed 1
+        assert want[:3] == [0x2e3ae8639566, 0x2508dc725c8a, 0xa279f7cf2ea3]
+    # continue from the returned state with a skip: one sequence
+    for skip in (0, 1, 11, 12, 13, 2**40 + 7, 2**64 - 1):
+        d2, st2, pos2 = rlx.rlxpp_host_generate(st, pos, p, skip, 15)
+        k = (pe + skip - 1) // 12 if skip else 0
+        Xs = pow(A, k, M) * Xe % M
+        ps = pe + skip - 12 * k
+        want2, X2, p2 = _py_stream(Xs, ps, A, 15)
+        assert [int(v * 2.0**48) for v in d2] == want2 and to_int(st2) == X2 and pos2 == p2
+    # non-canonical input (>= m) is reduced; the zero state is a fixed point with all draws 0.0
+    d3, st3, _ = rlx.rlxpp_host_generate(_limbs(M + 5), 12, p, 0, 3)
+    assert [int(v * 2.0**48) for v in d3] == _py_stream(5, 12, A, 3)[0]
+    d4, st4, _ = rlx.rlxpp_host_generate(_limbs(0), 3, p, 0, 20)
+    assert not d4.any() and to_int(st4) == 0
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_host_generate(_limbs(1), 13, p, 0, 1)
