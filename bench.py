@@ -191,6 +191,9 @@ def main():
                     help="engine of the LCG advance (include/rlxpp.h): tensor-core GEMM (default) or IMAD.WIDE")
     ap.add_argument("--layout", default="interleaved", choices=["interleaved", "stream_major"],
                     help="cfg3 / cfg4 output layout (BASELINE cfg3 names the interleaved one; stream_major is context)")
+    ap.add_argument("--output", default="f64", choices=["f64", "u48", "f32"],
+                    help="cfg3 / cfg4: what a 48-bit draw is stored as (SURVEY 8f-2): the double (BASELINE), the integer, "
+                         "or its two 24-bit floats; `value` stays in 48-bit draws per second")
     ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
@@ -236,8 +239,18 @@ def main():
         kernel = (f"tc_generate_kernel<{args.layout}, aligned>" if umma
                   else f"generate_kernel<Fixed<2048>, {args.layout}, aligned>")
 
+        if args.output == "u48":
+            out = out.view(torch.int64)
+        elif args.output == "f32":
+            out = out.view(torch.float32)
+
         def step():
-            rlx.rlxpp_generate_doubles(h, out, n_per, lay)
+            if args.output == "u48":
+                rlx.rlxpp_generate_u48(h, out, n_per, lay)
+            elif args.output == "f32":
+                rlx.rlxpp_generate_floats(h, out, 2 * n_per, lay)
+            else:
+                rlx.rlxpp_generate_doubles(h, out, n_per, lay)
     elif args.workload == "cfg5":
         h = rlx.rlxpp_create(n_streams, first_seed, p)
         sk = torch.from_numpy(inputs.cfg5_skip_distances(n_streams).view(np.int64)).cuda()
@@ -358,7 +371,7 @@ def main():
 
     # ---------------------------------------------------------------- the other engine, same workload (context)
     compare = None
-    if not args.no_compare and args.workload != "devapi":
+    if not args.no_compare and args.workload != "devapi" and args.output == "f64":
         other = "imad" if umma else "umma"
         rlx.rlxpp_set_engine(engines[other])
         step()
@@ -397,7 +410,7 @@ def main():
 
     # ---------------------------------------------------------------- end to end (host buffers)
     e2e = None
-    if not args.no_e2e and args.workload in ("cfg3", "cfg4", "cfg5"):
+    if not args.no_e2e and args.workload in ("cfg3", "cfg4", "cfg5") and args.output == "f64":
         if h is not None:
             rlx.rlxpp_destroy(h)
             h = None
@@ -451,7 +464,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": ("u8 x u8 -> s32 (tcgen05.mma kind::i8) + u32 limbs -> f64" if umma
                       else "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64"), "data": "synthetic",
-            "config": {"workload": args.workload, "engine": args.engine, "layout": args.layout, "description": desc, "n_streams_per_gpu": n_streams,
+            "config": {"workload": args.workload, "engine": args.engine, "layout": args.layout, "output": args.output, "description": desc, "n_streams_per_gpu": n_streams,
                        "doubles_per_stream": n_per, "p": p, "l2": "output per step (12.9 GB) exceeds L2; no flush needed"
                        if args.workload in ("cfg3", "cfg4") else "compute-bound; working set is registers",
                        "parallelism": f"streams sharded over {world} GPU(s), no collective"},
