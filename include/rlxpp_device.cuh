@@ -55,29 +55,110 @@ __host__ __device__ __forceinline__ constexpr u32 k240_limb(int j) {
 }
 
 // ------------------------------------------------------------------ generic product
-// multiply9x9 (sec. 2.1) on 32-bit limbs, column by column: "For every 64 bit in the
-// output, there are up to 9 contributing pairs ... The lower 64 bits of the sum constitutes
-// one entry of the output, while the rest is propagated to the next entry" -- here with
-// 32-bit entries and up to 18 pairs per column (device code multiplies 32-bit values).
-__device__ __forceinline__ void mul18x18(const u32 (&x)[18], const u32 (&y)[18], u32 (&z)[36]) {
-  u64 acc = 0;  // low 64 bits of the running column sum
-  u32 ovf = 0;  // bits 64.. of it
-#pragma unroll
-  for (int k = 0; k < 35; k++) {
-#pragma unroll
-    for (int i = 0; i < 18; i++) {
-      const int j = k - i;
-      if (j >= 0 && j < 18) {
-        const u64 p = (u64)x[i] * y[j];
-        acc += p;
-        ovf += (acc < p);  // P:134-137 Listing 4: branch-free carry
-      }
+// multiply9x9 (sec. 2.1): the 1152-bit schoolbook product, here on 32-bit limbs
+// (device code multiplies 32-bit values): 18 x 18 = 324 products 32x32->64.
+// Row by row with two interleaved sets of 64-bit accumulators, E[w] at 32-bit columns (2w, 2w + 1)
+// and O[w] at columns (2w + 1, 2w + 2): the product x_i y_j belongs to column i + j, so row i feeds
+// nine consecutive accumulators of each set through one carry chain (ptxas fuses every
+// mul.wide.u32 + add(c).cc.u64 into ONE IMAD.WIDE.U32.X: 324 instructions for the 324 products).
+// After rows 0..i each set is < 2^(32 (i + 19)): the carry out of a chain either lands in an
+// accumulator that holds less than 2^32 (added, cannot overflow) or is zero (chain already ends at
+// that bound) -- no carry ever ripples further.
+template <int I, bool ODD>  // one chain of row I: the products at even (ODD = false) or odd columns
+struct MulChain {
+  static constexpr int kJ0 = ODD ? ((I + 1) & 1) : (I & 1);  // first j of the chain (j advances by 2)
+  static constexpr int kW0 = ODD ? (I + kJ0 - 1) / 2 : (I + kJ0) / 2;
+  static constexpr bool kTail = kJ0 == 0;                     // carry out goes to accumulator kW0 + 9
+  static __device__ __forceinline__ void run(u64 (&acc)[18], u32 xi, const u32 (&y)[18]) {
+    if (kTail) {
+      asm("{\n\t.reg .u64 t;\n\t"
+          "mul.wide.u32 t, %10, %11; add.cc.u64  %0, %0, t;\n\t"
+          "mul.wide.u32 t, %10, %12; addc.cc.u64 %1, %1, t;\n\t"
+          "mul.wide.u32 t, %10, %13; addc.cc.u64 %2, %2, t;\n\t"
+          "mul.wide.u32 t, %10, %14; addc.cc.u64 %3, %3, t;\n\t"
+          "mul.wide.u32 t, %10, %15; addc.cc.u64 %4, %4, t;\n\t"
+          "mul.wide.u32 t, %10, %16; addc.cc.u64 %5, %5, t;\n\t"
+          "mul.wide.u32 t, %10, %17; addc.cc.u64 %6, %6, t;\n\t"
+          "mul.wide.u32 t, %10, %18; addc.cc.u64 %7, %7, t;\n\t"
+          "mul.wide.u32 t, %10, %19; addc.cc.u64 %8, %8, t;\n\t"
+          "addc.u64 %9, %9, 0;\n\t"
+          "}"
+          : "+l"(acc[kW0]), "+l"(acc[kW0 + 1]), "+l"(acc[kW0 + 2]), "+l"(acc[kW0 + 3]), "+l"(acc[kW0 + 4]),
+            "+l"(acc[kW0 + 5]), "+l"(acc[kW0 + 6]), "+l"(acc[kW0 + 7]), "+l"(acc[kW0 + 8]),
+            "+l"(acc[kW0 + 9 < 18 ? kW0 + 9 : 17])
+          : "r"(xi), "r"(y[kJ0]), "r"(y[kJ0 + 2]), "r"(y[kJ0 + 4]), "r"(y[kJ0 + 6]), "r"(y[kJ0 + 8]), "r"(y[kJ0 + 10]),
+            "r"(y[kJ0 + 12]), "r"(y[kJ0 + 14]), "r"(y[kJ0 + 16]));
+    } else {
+      asm("{\n\t.reg .u64 t;\n\t"
+          "mul.wide.u32 t, %9, %10; add.cc.u64  %0, %0, t;\n\t"
+          "mul.wide.u32 t, %9, %11; addc.cc.u64 %1, %1, t;\n\t"
+          "mul.wide.u32 t, %9, %12; addc.cc.u64 %2, %2, t;\n\t"
+          "mul.wide.u32 t, %9, %13; addc.cc.u64 %3, %3, t;\n\t"
+          "mul.wide.u32 t, %9, %14; addc.cc.u64 %4, %4, t;\n\t"
+          "mul.wide.u32 t, %9, %15; addc.cc.u64 %5, %5, t;\n\t"
+          "mul.wide.u32 t, %9, %16; addc.cc.u64 %6, %6, t;\n\t"
+          "mul.wide.u32 t, %9, %17; addc.cc.u64 %7, %7, t;\n\t"
+          "mul.wide.u32 t, %9, %18; addc.u64    %8, %8, t;\n\t"
+          "}"
+          : "+l"(acc[kW0]), "+l"(acc[kW0 + 1]), "+l"(acc[kW0 + 2]), "+l"(acc[kW0 + 3]), "+l"(acc[kW0 + 4]),
+            "+l"(acc[kW0 + 5]), "+l"(acc[kW0 + 6]), "+l"(acc[kW0 + 7]), "+l"(acc[kW0 + 8])
+          : "r"(xi), "r"(y[kJ0]), "r"(y[kJ0 + 2]), "r"(y[kJ0 + 4]), "r"(y[kJ0 + 6]), "r"(y[kJ0 + 8]), "r"(y[kJ0 + 10]),
+            "r"(y[kJ0 + 12]), "r"(y[kJ0 + 14]), "r"(y[kJ0 + 16]));
     }
-    z[k] = (u32)acc;
-    acc = (acc >> 32) | ((u64)ovf << 32);
-    ovf = 0;
   }
-  z[35] = (u32)acc;
+};
+template <int I>
+struct MulRows {
+  static __device__ __forceinline__ void run(u64 (&E)[18], u64 (&O)[18], const u32 (&x)[18], const u32 (&y)[18]) {
+    MulChain<I, false>::run(E, x[I], y);
+    MulChain<I, true>::run(O, x[I], y);
+    MulRows<I + 1>::run(E, O, x, y);
+  }
+};
+template <>
+struct MulRows<18> {
+  static __device__ __forceinline__ void run(u64 (&)[18], u64 (&)[18], const u32 (&)[18], const u32 (&)[18]) {}
+};
+
+__device__ __forceinline__ void mul18x18(const u32 (&x)[18], const u32 (&y)[18], u32 (&z)[36]) {
+  u64 E[18], O[18];
+#pragma unroll
+  for (int w = 0; w < 18; w++) { E[w] = 0; O[w] = 0; }
+  MulRows<0>::run(E, O, x, y);
+  // Z = E + (O << 32): T[w] = columns (2w, 2w + 1) of O << 32 = (high half of O[w - 1], low half of O[w])
+  u64 T[18], Z[18];
+  T[0] = O[0] << 32;
+#pragma unroll
+  for (int w = 1; w < 18; w++) T[w] = (O[w - 1] >> 32) | (O[w] << 32);
+  asm("add.cc.u64 %0, %18, %36;\n\t"
+      "addc.cc.u64 %1, %19, %37;\n\t"
+      "addc.cc.u64 %2, %20, %38;\n\t"
+      "addc.cc.u64 %3, %21, %39;\n\t"
+      "addc.cc.u64 %4, %22, %40;\n\t"
+      "addc.cc.u64 %5, %23, %41;\n\t"
+      "addc.cc.u64 %6, %24, %42;\n\t"
+      "addc.cc.u64 %7, %25, %43;\n\t"
+      "addc.cc.u64 %8, %26, %44;\n\t"
+      "addc.cc.u64 %9, %27, %45;\n\t"
+      "addc.cc.u64 %10, %28, %46;\n\t"
+      "addc.cc.u64 %11, %29, %47;\n\t"
+      "addc.cc.u64 %12, %30, %48;\n\t"
+      "addc.cc.u64 %13, %31, %49;\n\t"
+      "addc.cc.u64 %14, %32, %50;\n\t"
+      "addc.cc.u64 %15, %33, %51;\n\t"
+      "addc.cc.u64 %16, %34, %52;\n\t"
+      "addc.u64 %17, %35, %53;"
+      : "=l"(Z[0]), "=l"(Z[1]), "=l"(Z[2]), "=l"(Z[3]), "=l"(Z[4]), "=l"(Z[5]), "=l"(Z[6]), "=l"(Z[7]), "=l"(Z[8]),
+        "=l"(Z[9]), "=l"(Z[10]), "=l"(Z[11]), "=l"(Z[12]), "=l"(Z[13]), "=l"(Z[14]), "=l"(Z[15]), "=l"(Z[16]), "=l"(Z[17])
+      : "l"(E[0]), "l"(E[1]), "l"(E[2]), "l"(E[3]), "l"(E[4]), "l"(E[5]), "l"(E[6]), "l"(E[7]), "l"(E[8]), "l"(E[9]),
+        "l"(E[10]), "l"(E[11]), "l"(E[12]), "l"(E[13]), "l"(E[14]), "l"(E[15]), "l"(E[16]), "l"(E[17]), "l"(T[0]),
+        "l"(T[1]), "l"(T[2]), "l"(T[3]), "l"(T[4]), "l"(T[5]), "l"(T[6]), "l"(T[7]), "l"(T[8]), "l"(T[9]), "l"(T[10]),
+        "l"(T[11]), "l"(T[12]), "l"(T[13]), "l"(T[14]), "l"(T[15]), "l"(T[16]), "l"(T[17]));
+#pragma unroll
+  for (int w = 0; w < 18; w++) {
+    z[2 * w] = (u32)Z[w];
+    z[2 * w + 1] = (u32)(Z[w] >> 32);
+  }
 }
 
 // x >= m ?
