@@ -32,6 +32,7 @@ IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles 
 
 WORKLOADS = {
     # name: (streams, doubles per stream, p, description)
+    "cfg1": (1024, 384, 2048, "BASELINE configs[0]: 1,024 streams x 384 doubles, p=2048, stream-major (launch-latency bound: 8 CTAs)"),
     "cfg3": (1 << 20, 1536, 2048, "BASELINE configs[2]: 2^20 streams x 1536 doubles, p=2048, interleaved, 12.9 GB/step"),
     "cfg4": (1 << 18, 6144, 2048, "BASELINE configs[3] at p=2048: 2^18 streams x 6144 doubles, interleaved, 12.9 GB/step"),
     "cfg5": (1 << 18, 49152, 2048, "BASELINE configs[4]: 2^18 streams, random 64-bit skips, 49152 doubles fused to sum/sumsq"),
@@ -230,7 +231,9 @@ def main():
     stream = torch.cuda.current_stream()
 
     # ---------------------------------------------------------------- set up the step
-    if args.workload in ("cfg3", "cfg4"):
+    if args.workload == "cfg1":
+        args.layout = "stream_major"
+    if args.workload in ("cfg1", "cfg3", "cfg4"):
         h = rlx.rlxpp_create(n_streams, first_seed, p)
         out = torch.empty((n_per, n_streams), dtype=torch.float64, device="cuda")
         units = n_streams * n_per
@@ -320,14 +323,14 @@ def main():
     imad_achieved = units * IMAD_PER_DOUBLE / (kernel_ms * 1e-3)
     hbm_achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
     roof_alu = imad_nominal / IMAD_PER_DOUBLE
-    roof_hbm = hbm_gbs * 1e9 / 8 if args.workload in ("cfg3", "cfg4") else float("inf")
+    roof_hbm = hbm_gbs * 1e9 / 8 if args.workload in ("cfg1", "cfg3", "cfg4") else float("inf")
     doubles_rate = units / (kernel_ms * 1e-3)
     alu = {"achieved": imad_achieved / 1e9, "peak": imad_nominal / 1e9, "unit": "GIMAD/s", "frac": imad_achieved / imad_nominal,
            "model": "324 products 32x32->64 per advance (27 per double) whatever the engine; peak = "
                     f"{SM_COUNT} SMs x {IMAD_LANES_PER_CLK_SM} IMAD lanes/clk x {sm_max_mhz:.0f} MHz"}
     hbm = {"achieved": hbm_achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_achieved / hbm_gbs,
            "algorithmic_bytes_per_launch": alg_bytes}
-    stores = args.workload in ("cfg3", "cfg4")
+    stores = args.workload in ("cfg1", "cfg3", "cfg4")
     # The bound that binds: with the UMMA engine the products run on the tensor pipe, so a workload
     # that stores its doubles is bound by HBM writes; the IMAD engine and the store-free workloads
     # are bound by integer issue (reported against the 324-product model, north_star).
@@ -466,7 +469,9 @@ def main():
                       else "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64"), "data": "synthetic",
             "config": {"workload": args.workload, "engine": args.engine, "layout": args.layout, "output": args.output, "description": desc, "n_streams_per_gpu": n_streams,
                        "doubles_per_stream": n_per, "p": p, "l2": "output per step (12.9 GB) exceeds L2; no flush needed"
-                       if args.workload in ("cfg3", "cfg4") else "compute-bound; working set is registers",
+                       if args.workload in ("cfg3", "cfg4") else ("3 MB of output: L2-resident, launch-latency bound"
+                                                                  if args.workload == "cfg1" else
+                                                                  "compute-bound; working set is registers"),
                        "parallelism": f"streams sharded over {world} GPU(s), no collective"},
             "lcg_advances_per_s": value / 12.0,
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
