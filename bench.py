@@ -190,6 +190,8 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--engine", default="umma", choices=["umma", "imad"],
                     help="engine of the LCG advance (include/rlxpp.h): tensor-core GEMM (default) or IMAD.WIDE")
+    ap.add_argument("--p", type=int, default=None,
+                    help="luxury level (default: the workload's, 2048); BASELINE configs[3] sweeps 24, 389, 1024, 2048")
     ap.add_argument("--layout", default="interleaved", choices=["interleaved", "stream_major"],
                     help="cfg3 / cfg4 output layout (BASELINE cfg3 names the interleaved one; stream_major is context)")
     ap.add_argument("--output", default="f64", choices=["f64", "u48", "f32"],
@@ -224,6 +226,8 @@ def main():
     umma = args.engine == "umma" and args.workload != "devapi"  # the device API advances with IMADs per thread
 
     n_streams, n_per, p, desc = WORKLOADS[args.workload]
+    if args.p:
+        p = args.p
     # weak scaling: the job has world x n_streams streams, rank g owns the contiguous range g
     first_stream, my_streams = shard.stream_range(rank, world, world * n_streams)
     assert my_streams == n_streams
@@ -240,7 +244,7 @@ def main():
         alg_bytes = units * 8 + 2 * 80 * n_streams  # doubles written + state read and written back
         lay = rlx.RLXPP_INTERLEAVED if args.layout == "interleaved" else rlx.RLXPP_STREAM_MAJOR
         kernel = (f"tc_generate_kernel<{args.layout}, aligned>" if umma
-                  else f"generate_kernel<Fixed<2048>, {args.layout}, aligned>")
+                  else f"generate_kernel<Fixed<{p}>, {args.layout}, aligned>")
 
         if args.output == "u48":
             out = out.view(torch.int64)
@@ -262,7 +266,7 @@ def main():
         Q = torch.empty(n_streams, dtype=torch.float64, device="cuda")
         units = n_streams * n_per
         alg_bytes = (2 * 80 + 16) * n_streams
-        kernel = "tc_generate_kernel<reduce, unaligned>" if umma else "generate_kernel<Fixed<2048>, reduce, unaligned>"
+        kernel = "tc_generate_kernel<reduce, unaligned>" if umma else f"generate_kernel<Fixed<{p}>, reduce, unaligned>"
 
         def step():
             rlx.rlxpp_generate_reduce(h, S, Q, n_per)
@@ -285,7 +289,7 @@ def main():
         reps = n_per
         units = n_streams * reps * 12
         alg_bytes = 144 * n_streams
-        kernel = "tc_advance_states_kernel<AoS>" if umma else "advance_states_kernel<Fixed<2048>, AoS>"
+        kernel = "tc_advance_states_kernel<AoS>" if umma else f"advance_states_kernel<Fixed<{p}>, AoS>"
 
         def step():
             rlx.rlxpp_advance_states(states, n_streams, p, reps, rlx.RLXPP_AOS)
