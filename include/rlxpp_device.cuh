@@ -182,51 +182,138 @@ __device__ __forceinline__ void sub_m(u32 (&x)[18]) {
   for (int j = 8; j < 18; j++) x[j] = 0;
 }
 
+// value = r + k 2^576 (k small, signed)  ->  r + k (2^240 - 1), returned again as (r, new k).
+// k (2^240 - 1) as an 18-limb two's-complement constant: limb 0 = -k, limbs 1..6 = all ones if k > 0,
+// limb 7 = (k << 16) - [k > 0], limbs 8..17 = all ones if k < 0 (sign extension).
+__device__ __forceinline__ int fold_carry(u32 (&r)[18], int k) {
+  const u32 c0 = (u32)(-k), sp = k > 0 ? 0xFFFFFFFFu : 0u, c7 = ((u32)k << 16) - (k > 0 ? 1u : 0u),
+            ng = k < 0 ? 0xFFFFFFFFu : 0u;
+  u32 cout;
+  asm(
+      "add.cc.u32 %0, %0, %19;\n\t"
+      "addc.cc.u32 %1, %1, %20;\n\t"
+      "addc.cc.u32 %2, %2, %20;\n\t"
+      "addc.cc.u32 %3, %3, %20;\n\t"
+      "addc.cc.u32 %4, %4, %20;\n\t"
+      "addc.cc.u32 %5, %5, %20;\n\t"
+      "addc.cc.u32 %6, %6, %20;\n\t"
+      "addc.cc.u32 %7, %7, %21;\n\t"
+      "addc.cc.u32 %8, %8, %22;\n\t"
+      "addc.cc.u32 %9, %9, %22;\n\t"
+      "addc.cc.u32 %10, %10, %22;\n\t"
+      "addc.cc.u32 %11, %11, %22;\n\t"
+      "addc.cc.u32 %12, %12, %22;\n\t"
+      "addc.cc.u32 %13, %13, %22;\n\t"
+      "addc.cc.u32 %14, %14, %22;\n\t"
+      "addc.cc.u32 %15, %15, %22;\n\t"
+      "addc.cc.u32 %16, %16, %22;\n\t"
+      "addc.cc.u32 %17, %17, %22;\n\t"
+      "addc.u32 %18, 0, 0;"
+      : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15]), "+r"(r[16]), "+r"(r[17]), "=r"(cout)
+      : "r"(c0), "r"(sp), "r"(c7), "r"(ng));
+  return (int)cout - (k < 0 ? 1 : 0);
+}
+
 // mod_m (sec. 2.2): remainder of a 1152-bit value modulo m "using additions,
 // subtractions, and bit shifts" plus the "fix to ensure that the result is smaller than m
-// in all cases".  Reading c-9:  z = lo + hi 2^576, hi = t1 2^336 + t0, u = t0 + t1,
-//   z == lo - hi - t1 + (u mod 2^336) 2^240 + (u >> 336)(2^240 - 1)   (mod m)
-// summed limb by limb with a signed carry; the final carry k is folded again as
-// k (2^240 - 1), and m is subtracted once if the result is still >= m.
+// in all cases".  Reading c-9:  z = lo + hi 2^576, hi = t1 2^336 + t0, u = t0 + t1 (337 bits),
+//   z == lo + u 2^240 - hi - t1   (mod m)        [hi 2^576 == hi (2^240 - 1), t1 2^576 likewise]
+// evaluated as P - N with P = lo + u 2^240 and N = hi + t1 (19 limbs each, PTX carry chains); what
+// lies above 2^576 is a small signed k, folded again as k (2^240 - 1); m is subtracted once if the
+// result is still >= m.
 __device__ __forceinline__ void mod_m36(const u32 (&z)[36], u32 (&r)[18]) {
-  u32 t1[8];
+  u32 t1[8];  // hi >> 336
 #pragma unroll
-  for (int j = 0; j < 7; j++) t1[j] = (z[28 + j] >> 16) | (z[29 + j] << 16);
+  for (int j = 0; j < 7; j++) t1[j] = __funnelshift_r(z[28 + j], z[29 + j], 16);
   t1[7] = z[35] >> 16;
-  u32 u[11];
-  u64 c = 0;
+  u32 u[11];  // u = t0 + t1 < 2^337 (u[10] < 2^17)
+  asm(
+      "add.cc.u32 %0, %11, %22;\n\t"
+      "addc.cc.u32 %1, %12, %23;\n\t"
+      "addc.cc.u32 %2, %13, %24;\n\t"
+      "addc.cc.u32 %3, %14, %25;\n\t"
+      "addc.cc.u32 %4, %15, %26;\n\t"
+      "addc.cc.u32 %5, %16, %27;\n\t"
+      "addc.cc.u32 %6, %17, %28;\n\t"
+      "addc.cc.u32 %7, %18, %29;\n\t"
+      "addc.cc.u32 %8, %19, 0;\n\t"
+      "addc.cc.u32 %9, %20, 0;\n\t"
+      "addc.u32 %10, %21, 0;"
+      : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]), "=r"(u[8]), "=r"(u[9]), "=r"(u[10])
+      : "r"(z[18]), "r"(z[19]), "r"(z[20]), "r"(z[21]), "r"(z[22]), "r"(z[23]), "r"(z[24]), "r"(z[25]), "r"(z[26]), "r"(z[27]), "r"(z[28] & 0xFFFFu), "r"(t1[0]), "r"(t1[1]), "r"(t1[2]), "r"(t1[3]), "r"(t1[4]), "r"(t1[5]), "r"(t1[6]), "r"(t1[7]));
+  // P = lo + u 2^240 (19 limbs: limbs 0..6 are lo's), N = hi + t1 (19 limbs)
+  u32 ush[12];  // limbs 7..18 of u << 240
+  ush[0] = u[0] << 16;
 #pragma unroll
-  for (int j = 0; j < 11; j++) {
-    const u64 s = (u64)(j < 10 ? z[18 + j] : (z[28] & 0xFFFFu)) + (j < 8 ? t1[j] : 0u) + c;
-    u[j] = (u32)s;
-    c = s >> 32;
-  }
-  const u32 ubit = u[10] >> 16;  // u >> 336
-  u[10] &= 0xFFFFu;              // u mod 2^336
-  i64 carry = 0;
+  for (int j = 1; j < 11; j++) ush[j] = __funnelshift_l(u[j - 1], u[j], 16);
+  ush[11] = u[10] >> 16;
+  u32 pp[18], p18, nn[18], n18, bw;
 #pragma unroll
-  for (int j = 0; j < 18; j++) {
-    u32 ush = 0;  // limb j of (u mod 2^336) << 240
-    if (j == 7) ush = u[0] << 16;
-    else if (j > 7) ush = (u[j - 7] << 16) | (u[j - 8] >> 16);
-    const i64 s = (i64)z[j] - (i64)z[18 + j] - (i64)(j < 8 ? t1[j] : 0u) + (i64)ush +
-                  (i64)(ubit ? k240_limb(j) : 0u) + carry;
-    r[j] = (u32)s;
-    carry = s >> 32;
-  }
-  // value = r + carry 2^576 == r + carry (2^240 - 1); by the bound in c-9 |carry| <= 1 and one
-  // fold suffices; a second pass (normally with 0) keeps this exact even if it did not.
-#pragma unroll
-  for (int pass = 0; pass < 2; pass++) {
-    const i64 k = carry;
-    carry = 0;
-#pragma unroll
-    for (int j = 0; j < 18; j++) {
-      const i64 s = (i64)r[j] + k * (i64)k240_limb(j) + carry;
-      r[j] = (u32)s;
-      carry = s >> 32;
-    }
-  }
+  for (int j = 0; j < 7; j++) pp[j] = z[j];
+  asm(
+      "add.cc.u32 %0, %12, %23;\n\t"
+      "addc.cc.u32 %1, %13, %24;\n\t"
+      "addc.cc.u32 %2, %14, %25;\n\t"
+      "addc.cc.u32 %3, %15, %26;\n\t"
+      "addc.cc.u32 %4, %16, %27;\n\t"
+      "addc.cc.u32 %5, %17, %28;\n\t"
+      "addc.cc.u32 %6, %18, %29;\n\t"
+      "addc.cc.u32 %7, %19, %30;\n\t"
+      "addc.cc.u32 %8, %20, %31;\n\t"
+      "addc.cc.u32 %9, %21, %32;\n\t"
+      "addc.cc.u32 %10, %22, %33;\n\t"
+      "addc.u32 %11, %34, 0;"
+      : "=r"(pp[7]), "=r"(pp[8]), "=r"(pp[9]), "=r"(pp[10]), "=r"(pp[11]), "=r"(pp[12]), "=r"(pp[13]), "=r"(pp[14]), "=r"(pp[15]), "=r"(pp[16]), "=r"(pp[17]), "=r"(p18)
+      : "r"(z[7]), "r"(z[8]), "r"(z[9]), "r"(z[10]), "r"(z[11]), "r"(z[12]), "r"(z[13]), "r"(z[14]), "r"(z[15]), "r"(z[16]), "r"(z[17]), "r"(ush[0]), "r"(ush[1]), "r"(ush[2]), "r"(ush[3]), "r"(ush[4]), "r"(ush[5]), "r"(ush[6]), "r"(ush[7]), "r"(ush[8]), "r"(ush[9]), "r"(ush[10]), "r"(ush[11]));
+  asm(
+      "add.cc.u32 %0, %19, %37;\n\t"
+      "addc.cc.u32 %1, %20, %38;\n\t"
+      "addc.cc.u32 %2, %21, %39;\n\t"
+      "addc.cc.u32 %3, %22, %40;\n\t"
+      "addc.cc.u32 %4, %23, %41;\n\t"
+      "addc.cc.u32 %5, %24, %42;\n\t"
+      "addc.cc.u32 %6, %25, %43;\n\t"
+      "addc.cc.u32 %7, %26, %44;\n\t"
+      "addc.cc.u32 %8, %27, 0;\n\t"
+      "addc.cc.u32 %9, %28, 0;\n\t"
+      "addc.cc.u32 %10, %29, 0;\n\t"
+      "addc.cc.u32 %11, %30, 0;\n\t"
+      "addc.cc.u32 %12, %31, 0;\n\t"
+      "addc.cc.u32 %13, %32, 0;\n\t"
+      "addc.cc.u32 %14, %33, 0;\n\t"
+      "addc.cc.u32 %15, %34, 0;\n\t"
+      "addc.cc.u32 %16, %35, 0;\n\t"
+      "addc.cc.u32 %17, %36, 0;\n\t"
+      "addc.u32 %18, 0, 0;"
+      : "=r"(nn[0]), "=r"(nn[1]), "=r"(nn[2]), "=r"(nn[3]), "=r"(nn[4]), "=r"(nn[5]), "=r"(nn[6]), "=r"(nn[7]), "=r"(nn[8]), "=r"(nn[9]), "=r"(nn[10]), "=r"(nn[11]), "=r"(nn[12]), "=r"(nn[13]), "=r"(nn[14]), "=r"(nn[15]), "=r"(nn[16]), "=r"(nn[17]), "=r"(n18)
+      : "r"(z[18]), "r"(z[19]), "r"(z[20]), "r"(z[21]), "r"(z[22]), "r"(z[23]), "r"(z[24]), "r"(z[25]), "r"(z[26]), "r"(z[27]), "r"(z[28]), "r"(z[29]), "r"(z[30]), "r"(z[31]), "r"(z[32]), "r"(z[33]), "r"(z[34]), "r"(z[35]), "r"(t1[0]), "r"(t1[1]), "r"(t1[2]), "r"(t1[3]), "r"(t1[4]), "r"(t1[5]), "r"(t1[6]), "r"(t1[7]));
+  asm(
+      "sub.cc.u32 %0, %19, %37;\n\t"
+      "subc.cc.u32 %1, %20, %38;\n\t"
+      "subc.cc.u32 %2, %21, %39;\n\t"
+      "subc.cc.u32 %3, %22, %40;\n\t"
+      "subc.cc.u32 %4, %23, %41;\n\t"
+      "subc.cc.u32 %5, %24, %42;\n\t"
+      "subc.cc.u32 %6, %25, %43;\n\t"
+      "subc.cc.u32 %7, %26, %44;\n\t"
+      "subc.cc.u32 %8, %27, %45;\n\t"
+      "subc.cc.u32 %9, %28, %46;\n\t"
+      "subc.cc.u32 %10, %29, %47;\n\t"
+      "subc.cc.u32 %11, %30, %48;\n\t"
+      "subc.cc.u32 %12, %31, %49;\n\t"
+      "subc.cc.u32 %13, %32, %50;\n\t"
+      "subc.cc.u32 %14, %33, %51;\n\t"
+      "subc.cc.u32 %15, %34, %52;\n\t"
+      "subc.cc.u32 %16, %35, %53;\n\t"
+      "subc.cc.u32 %17, %36, %54;\n\t"
+      "subc.u32 %18, 0, 0;"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(bw)
+      : "r"(pp[0]), "r"(pp[1]), "r"(pp[2]), "r"(pp[3]), "r"(pp[4]), "r"(pp[5]), "r"(pp[6]), "r"(pp[7]), "r"(pp[8]), "r"(pp[9]), "r"(pp[10]), "r"(pp[11]), "r"(pp[12]), "r"(pp[13]), "r"(pp[14]), "r"(pp[15]), "r"(pp[16]), "r"(pp[17]), "r"(nn[0]), "r"(nn[1]), "r"(nn[2]), "r"(nn[3]), "r"(nn[4]), "r"(nn[5]), "r"(nn[6]), "r"(nn[7]), "r"(nn[8]), "r"(nn[9]), "r"(nn[10]), "r"(nn[11]), "r"(nn[12]), "r"(nn[13]), "r"(nn[14]), "r"(nn[15]), "r"(nn[16]), "r"(nn[17]));
+  // z == r + k 2^576 with k = p18 - n18 - borrow in [-2, 2];  2^576 == 2^240 - 1:  fold k, then the
+  // carry of that fold (|k'| <= 1; by the bound in c-9 a second fold leaves none)
+  int k = (int)p18 - (int)n18 - (int)(bw & 1u);
+  k = fold_carry(r, k);
+  if (k != 0) k = fold_carry(r, k);
   if (ge_m(r)) sub_m(r);  // the fix: result < m
 }
 
