@@ -135,15 +135,19 @@ __device__ __forceinline__ void to_ranlux_fast(const u32 (&x)[18], u32 (&v)[18],
 // D6 (c-5, c-11): draw j of a block = bits [48 j, 48 j + 48) of V, as the double k 2^-48.
 // The 48 bits are placed in the mantissa of 2^4 (value 16 + k 2^-48, exact) and 16.0 is
 // subtracted (exact): one PRMT or two, one DADD; no int->float conversion instruction.
+// kexp = the high word of 16.0 (0x40300000), handed to the kernels as a launch PARAMETER so that it
+// sits in a register and the PRMT selectors are immediates: with both as literals ptxas puts the
+// selector in a register and re-materialises it for every draw (12 extra instructions per advance).
+constexpr u32 kExp16 = 0x40300000u;
 template <int J>
-__device__ __forceinline__ double draw_double(const u32 (&v)[18]) {
+__device__ __forceinline__ double draw_double(const u32 (&v)[18], u32 kexp) {
   u32 lo, hi;
   if (J % 2 == 0) {  // bits 48J.. start on a limb boundary: limbs 3J/2, 3J/2 + 1 (low half)
     lo = v[3 * J / 2];
-    hi = __byte_perm(v[3 * J / 2 + 1], 0x40300000u, 0x7610);
+    hi = __byte_perm(v[3 * J / 2 + 1], kexp, 0x7610);
   } else {  // start in the middle of limb (3J - 1)/2
     lo = __byte_perm(v[(3 * J - 1) / 2], v[(3 * J + 1) / 2], 0x5432);
-    hi = __byte_perm(v[(3 * J + 1) / 2], 0x40300000u, 0x7632);
+    hi = __byte_perm(v[(3 * J + 1) / 2], kexp, 0x7632);
   }
   return __hiloint2double((int)hi, (int)lo) - 16.0;
 }
