@@ -197,6 +197,8 @@ def main():
     ap.add_argument("--output", default="f64", choices=["f64", "u48", "f32"],
                     help="cfg3 / cfg4: what a 48-bit draw is stored as (SURVEY 8f-2): the double (BASELINE), the integer, "
                          "or its two 24-bit floats; `value` stays in 48-bit draws per second")
+    ap.add_argument("--chunks", type=int, default=0,
+                    help="UMMA engine: force the number of chunks per tile (rlxpp_set_chunks; 0 = the library decides)")
     ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
@@ -223,6 +225,7 @@ def main():
     rlx.load()
     engines = {"umma": rlx.RLXPP_ENGINE_UMMA, "imad": rlx.RLXPP_ENGINE_IMAD}
     rlx.rlxpp_set_engine(engines[args.engine])
+    rlx.rlxpp_set_chunks(args.chunks)
     umma = args.engine == "umma" and args.workload != "devapi"  # the device API advances with IMADs per thread
 
     n_streams, n_per, p, desc = WORKLOADS[args.workload]

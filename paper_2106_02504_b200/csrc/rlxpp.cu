@@ -929,13 +929,17 @@ static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_
   *chunk_len = n_per;
   const uint64_t blocks = n_per / 12;
   if (n_tiles <= slots || blocks < 32) return;
+  // a good plan fills >= 97 % of its last wave AND has >= 12 waves: CTAs do not run at equal speed when the
+  // kernel is HBM-bound, and finer items even that out (cfg4: 2 chunks 764, 4 chunks 793 G doubles/s at the
+  // same 98.8 % fill; profiles/ab_r01_sync.md)
   double best = 0.0;
   uint64_t best_c = 1;
   for (uint64_t c = 1; c <= 16 && blocks / c >= 16; c++) {
     const uint64_t items = n_tiles * c, waves = (items + slots - 1) / slots;
     const double eff = (double)items / (double)(waves * slots);
-    if (eff > best + 1e-9) { best = eff; best_c = c; }
-    if (eff >= 0.97) break;
+    const double score = eff - (waves < 12 ? 0.05 : 0.0);
+    if (score > best + 1e-9) { best = score; best_c = c; }
+    if (eff >= 0.97 && waves >= 12) break;
   }
   if (best_c == 1) return;
   const uint64_t len = ((blocks + best_c - 1) / best_c + 1) / 2 * 24;  // an even number of blocks (TMA store pairs)

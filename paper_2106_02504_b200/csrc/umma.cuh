@@ -29,6 +29,19 @@ __host__ __device__ constexpr u32 idesc_u8u8_s32(int M, int N) {
   return (2u << 4) | ((u32)(N >> 3) << 17) | ((u32)(M >> 4) << 24);
 }
 
+// One lane of the (converged) warp: true for exactly one of the lanes in the mask.
+__device__ __forceinline__ bool elect_one() {
+  u32 pred;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "elect.sync _|p, 0xFFFFFFFF;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t"
+      "}"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 // D[tmem] (+)= A[smem] * B[smem]^T, one CTA; issued by ONE thread on behalf of the CTA.
 __device__ __forceinline__ void mma_i8(u32 d_tmem, u64 adesc, u64 bdesc, u32 idesc, u32 accumulate) {
   asm volatile(
