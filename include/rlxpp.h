@@ -186,6 +186,13 @@ uint64_t rlxpp_launch_count(void);
  * Both time `iters` launches with CUDA events after a warm-up and report the best. */
 int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream);
 int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s, void* cuda_stream);
+/* The stream-major store pattern as the memory system sees it (no passage of the paper: it
+ * never writes draws to memory).  A persistent grid (the generate kernels' grid) in
+ * which every warp owns 32 rows of `pitch_bytes` at a time and writes one piece of `piece_bytes` of each of
+ * them per step; `rows` x pitch_bytes are allocated and freed inside the call.  rows: multiple of 32; piece
+ * and pitch: multiples of 16 bytes.  Returns the bytes/s of the best of `iters` launches after a warm-up. */
+int rlxpp_measure_hbm_write_pieces(uint64_t rows, uint64_t pitch_bytes, uint32_t piece_bytes, int iters, double* bytes_per_s,
+                                   void* cuda_stream);
 
 const char* rlxpp_last_error(void);
 const char* rlxpp_version(void);

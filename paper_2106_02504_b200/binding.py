@@ -66,6 +66,8 @@ _SIGNATURES = {
     "rlxpp_measure_imad_peak": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]),
     "rlxpp_measure_hbm_write_peak": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                                     ctypes.c_void_p]),
+    "rlxpp_measure_hbm_write_pieces": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int,
+                                                      ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]),
     "rlxpp_last_error": (ctypes.c_char_p, []),
     "rlxpp_version": (ctypes.c_char_p, []),
 }
@@ -286,6 +288,14 @@ def rlxpp_measure_hbm_write_peak(nbytes: int, iters: int = 5, cuda_stream=None) 
     out = ctypes.c_double(0.0)
     s = _current_stream() if cuda_stream is None else cuda_stream
     _check(load().rlxpp_measure_hbm_write_peak(nbytes, iters, ctypes.byref(out), s), "rlxpp_measure_hbm_write_peak")
+    return out.value
+
+
+def rlxpp_measure_hbm_write_pieces(rows: int, pitch_bytes: int, piece_bytes: int, iters: int = 3, cuda_stream=None) -> float:
+    out = ctypes.c_double(0.0)
+    s = _current_stream() if cuda_stream is None else cuda_stream
+    _check(load().rlxpp_measure_hbm_write_pieces(rows, pitch_bytes, piece_bytes, iters, ctypes.byref(out), s),
+           "rlxpp_measure_hbm_write_pieces")
     return out.value
 
 

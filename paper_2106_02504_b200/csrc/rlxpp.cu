@@ -391,71 +391,105 @@ namespace rlx {
 // Stream-major stores through shared memory and the TMA (S8 a-7a; north_star: "shared-memory
 // staging, or TMA bulk stores, so HBM writes are fully coalesced").  A thread's block is 96
 // contiguous bytes of ITS stream's row, so direct stores make every warp instruction touch 32 rows
-// (measured 287 G doubles/s, 36 % of the HBM peak).  Instead each warp parks the blocks of TWO
-// advances in shared memory as a dense [32 streams][24 doubles] box and one lane hands it to the
-// TMA: one cp.async.bulk.tensor.2d (SASS UTMASTG) per warp and pair of advances writes 32 row
-// segments of 192 bytes (six whole sectors); rows past the end of the launch are clipped by the
-// tensor map.  The even block of a pair fills the left half of every row, the odd one the right half
-// and sends the box; it is rewritten only after that copy has finished reading it
-// (cp.async.bulk.wait_group.read 0, a whole advance later).  A lone last block is sent with the
-// right half clipped by the tensor map (it can only be the end of the row: chunks are cut at even
-// block counts).  Measured 625 G doubles/s (78 % of the HBM peak; DRAM sees 192-byte pieces 12 KB apart).
-constexpr int kStageBoxCols = 24;
-constexpr int kStageWarpBytes = 32 * 192;
+// (measured 287 G doubles/s, 36 % of the HBM peak).  What the memory system wants is measured in
+// profiles/ab_r01_stream_major.md: row pieces that are 256 bytes long, 256-byte aligned and written by ONE
+// operation reach the interleaved layout's bandwidth; 96-, 128- or 192-byte pieces (or two 128-byte
+// halves from two operations) stop at 4.7 - 5.8 TB/s however they are fenced or buffered.
+// So each warp owns ONE box of [32 streams][32 doubles] in shared memory.  The 96 bytes of an advance
+// go where they fall in a cycle of 8 advances = 768 bytes = 3 boxes; an advance that straddles a box
+// end (phases 2 and 5) fills the box, one lane hands it to the TMA (cp.async.bulk.tensor.3d, SASS
+// UTMASTG) and the thread keeps the limbs of its remaining 4 or 8 draws in registers until the next
+// advance, which first waits for the copy to have read the box (cp.async.bulk.wait_group.read: one
+// whole advance of slack) and then stores them at the start of the box.
+// Tensor map: out[count][n_per] viewed as [count][n_per / 16][16 doubles] with a {16, 2, 32} box and
+// SWIZZLE_128B, so that one operation writes 32 x 256 contiguous bytes while the 16-byte chunks of a
+// row are XOR-swizzled in shared memory (2-way instead of 8-way bank conflicts on the st.shared.v2.f64;
+// a 2-D box with a 256-byte inner extent cannot be swizzled).  Rows past the end of the launch are
+// clipped by the tensor map.  Only whole cycles are staged: the last (n_per / 12) % 8 blocks of a row
+// are stored directly.
+constexpr u32 kStageWarpBytes = 32u * 256u;                    // one box
+constexpr u32 kStageCtaBytes = 4u * kStageWarpBytes + 1024u;   // dynamic shared memory of the staged kernels (+ alignment)
+constexpr u64 kStageCycle = 96;                                // draws per cycle of 8 advances
 struct StreamMajorStage {
-  u32 box;        // shared address of this warp's box
-  u32 wr;         // byte offset of this lane's row inside the box
+  u32 box;        // shared address of this warp's box (1,024-byte aligned: the swizzle works on address bits)
+  u32 rowbase;    // ... of this lane's 256-byte row
+  u32 rs;         // swizzle term of the row: ((2 lane) & 6) << 4
+  u32 q;          // phase: advance within the cycle
+  int col16;      // tensor coordinate (in units of 16 doubles) of the box being filled
+  int c1;         // tensor row of the warp's first stream
   const void* tmap;
   u32 kexp;       // exp16()
-  int c1;         // tensor coordinate of the warp's first stream (row)
-  __device__ __forceinline__ void init(uint8_t* stage, const void* tensor_map, u64 tile_first, u32 kexp_) {
+  u32 cv[18];     // limbs of the block whose last draws wait for the next box (only [6, 18) are ever live)
+  __device__ __forceinline__ void init(uint8_t* stage, const void* tensor_map, u64 tile_first, u32 kexp_, u64 t0) {
     const u32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    box = umma::smem_u32(stage) + warp * kStageWarpBytes;
-    wr = lane * (kStageBoxCols * 8u);
+    box = ((umma::smem_u32(stage) + 1023u) & ~1023u) + warp * kStageWarpBytes;
+    rowbase = box + lane * 256u;
+    rs = ((2u * lane) & 6u) << 4;
+    q = 0;
+    col16 = (int)(t0 / 16);
+    c1 = (int)(tile_first + warp * 32u);
     tmap = tensor_map;
     kexp = kexp_;
-    c1 = (int)(tile_first + warp * 32u);
   }
-  template <int OUT, int J>
+  // draws J, J + 1 of v to byte offset O of the lane's row.  The box is 64 lines of 128 bytes (line 2 r + h
+  // = half h of row r); SWIZZLE_128B stores 16-byte chunk c of a line at c ^ (line & 7) = c ^ h ^ ((2 r) & 6).
+  template <int OUT, int J, int O>
+  __device__ __forceinline__ void put2(const u32 (&v)[18]) {
+    constexpr u32 h = (u32)O >> 7, K = ((((u32)O >> 4) & 7u) ^ h) << 4;
+    const double a = draw_value<OUT, J>(v, kexp), b = draw_value<OUT, J + 1>(v, kexp);
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"((rowbase | (rs ^ K)) + h * 128u), "d"(a), "d"(b) : "memory");
+  }
+  template <int OUT, int J0, int J1, int O>
   struct Put {
-    static __device__ __forceinline__ void all(u32 dst, const u32 (&v)[18], u32 kexp) {
-      const double a = draw_value<OUT, J>(v, kexp), b = draw_value<OUT, J + 1>(v, kexp);
-      asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(dst + J * 8), "d"(a), "d"(b) : "memory");
-      Put<OUT, J + 2>::all(dst, v, kexp);
+    static __device__ __forceinline__ void all(StreamMajorStage& st, const u32 (&v)[18]) {
+      st.put2<OUT, J0, O>(v);
+      Put<OUT, J0 + 2, J1, O + 16>::all(st, v);
     }
   };
-  __device__ __forceinline__ void send(u32 src, int c0) {
-    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap), "r"(c0),
-                 "r"(c1), "r"(src)
-                 : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  __device__ __forceinline__ void wait_box() {  // whole warp: the last copy has read the box
+    if ((threadIdx.x & 31u) == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    __syncwarp();
   }
-  // whole-warp call; t = index of the block's first draw within the stream's row, blk = index of the
-  // block within the item, last = it is the item's last block
+  __device__ __forceinline__ void send() {  // whole warp: the box is full
+    umma::fence_proxy_async_smem();
+    __syncwarp();
+    if ((threadIdx.x & 31u) == 0) {
+      asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tmap), "r"(0),
+                   "r"(col16), "r"(c1), "r"(box)
+                   : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    col16 += 2;
+  }
+  template <int FROM>
+  __device__ __forceinline__ void keep(const u32 (&v)[18]) {
+#pragma unroll
+    for (int j = FROM; j < 18; j++) cv[j] = v[j];
+  }
+  // whole-warp call: the next block of the item (blocks come in whole cycles of 8)
   template <int OUT>
-  __device__ __forceinline__ void emit(const u32 (&v)[18], u64 t, u64 blk, bool last) {
-    const bool leader = (threadIdx.x & 31u) == 0;
-    const u32 half = (u32)(blk & 1u);
-    if (half == 0) {
-      if (leader) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-      __syncwarp();
+  __device__ __forceinline__ void emit(const u32 (&v)[18]) {
+    switch (q) {
+      case 0: wait_box(); Put<OUT, 0, 12, 0>::all(*this, v); break;
+      case 1: Put<OUT, 0, 12, 96>::all(*this, v); break;
+      case 2: Put<OUT, 0, 8, 192>::all(*this, v); send(); keep<12>(v); break;
+      case 3: wait_box(); Put<OUT, 8, 12, 0>::all(*this, cv); Put<OUT, 0, 12, 32>::all(*this, v); break;
+      case 4: Put<OUT, 0, 12, 128>::all(*this, v); break;
+      case 5: Put<OUT, 0, 4, 224>::all(*this, v); send(); keep<6>(v); break;
+      case 6: wait_box(); Put<OUT, 4, 12, 0>::all(*this, cv); Put<OUT, 0, 12, 64>::all(*this, v); break;
+      default: Put<OUT, 0, 12, 160>::all(*this, v); send(); break;
     }
-    Put<OUT, 0>::all(box + wr + half * 96u, v, kexp);
-    if (half == 1 || last) {
-      umma::fence_proxy_async_smem();
-      __syncwarp();
-      if (leader) send(box, (int)(t - half * 12u));
-    }
+    q = (q + 1u) & 7u;
   }
-  // before the boxes are reused by another item or the CTA exits
+  // before the box is reused by another item or the CTA exits
   __device__ __forceinline__ void drain() {
     if ((threadIdx.x & 31u) == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     __syncwarp();
   }
 };
-template <int OUT>
-struct StreamMajorStage::Put<OUT, 12> {
-  static __device__ __forceinline__ void all(u32, const u32 (&)[18], u32) {}
+template <int OUT, int J1, int O>
+struct StreamMajorStage::Put<OUT, J1, J1, O> {
+  static __device__ __forceinline__ void all(StreamMajorStage&, const u32 (&)[18]) {}
 };
 
 // ----------------------------------------------------------------------------- UMMA engine
@@ -479,7 +513,7 @@ template <int MODE, bool ALIGNED, int OUT = kF64>
 __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(const __grid_constant__ GenArgs a) {
   __shared__ tc::Smem smem;
   constexpr bool kStaged = MODE == kStoreStreamMajor && ALIGNED;
-  __shared__ __align__(128) uint8_t stage[kStaged ? 4 * kStageWarpBytes : 16];
+  extern __shared__ __align__(128) uint8_t stage[];  // kStageCtaBytes when kStaged, else none
   tc::Tile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
   tile.setup(smem, a.bmat);
   // the parameter form saves 12 instructions per advance and helps the ALU-bound fused kernel (+5 %); the
@@ -527,7 +561,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
     if (ALIGNED) {
       const u64 nblk = n / 12;
       StreamMajorStage sm;
-      if (kStaged) sm.init(stage, &a.tmap, (u64)tidx * tc::kTile, kexp);
+      if (kStaged) sm.init(stage, &a.tmap, (u64)tidx * tc::kTile, kexp, t0);
+      const u64 nstaged = nblk & ~(u64)7;  // whole cycles go through the TMA, the rest of a row is stored directly
       if (nblk > 0) tile.issue(x);
 #pragma unroll 1
       for (u64 b = 0; b < nblk; b++) {
@@ -536,7 +571,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         tc::reduce_z(z, x);
         if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
         to_ranlux_hot(x, v, c);
-        if (kStaged) sm.emit<OUT>(v, t0 + b * 12, b, b + 1 == nblk);
+        if (kStaged && b < nstaged) sm.emit<OUT>(v);
         else if (live) EmitBlock<0, MODE, OUT>::all(sink, v, b * 12);
       }
       if (kStaged) sm.drain();
@@ -793,6 +828,20 @@ __global__ void __launch_bounds__(256) hbm_write_kernel(uint4* __restrict__ out,
   for (u64 q = (u64)blockIdx.x * blockDim.x + threadIdx.x; q < n16; q += stride) __stcs(out + q, val);
 }
 
+// Store-pattern probe (rlxpp_measure_hbm_write_pieces): what a stream-major output looks like to the
+// memory system.  Every warp of a persistent grid owns 32 rows at a time and walks along them, writing
+// one piece of `piece16` x 16 bytes of each of its rows per step with full 128-bit stores.
+__global__ void __launch_bounds__(128, 4) hbm_write_pieces_kernel(uint4* __restrict__ out, u64 rows, u64 pitch16, u32 piece16) {
+  const u32 lane = threadIdx.x & 31u;
+  const u64 warp = (u64)blockIdx.x * 4 + (threadIdx.x >> 5), n_warps = (u64)gridDim.x * 4;
+  const uint4 v = make_uint4(0x3c3c3c3cu, 0x5a5a5a5au, (u32)warp, lane);
+  for (u64 g = warp; g < rows / 32; g += n_warps) {
+    uint4* base = out + g * 32 * pitch16;
+    for (u64 c = 0; c + piece16 <= pitch16; c += piece16)
+      for (u32 u = lane; u < 32u * piece16; u += 32u) __stcs(base + (u64)(u / piece16) * pitch16 + c + u % piece16, v);
+  }
+}
+
 // ----------------------------------------------------------------------------- host side
 struct Tables {
   uint32_t p = 0;
@@ -942,7 +991,7 @@ static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_
     if (eff >= 0.97 && waves >= 12) break;
   }
   if (best_c == 1) return;
-  const uint64_t len = ((blocks + best_c - 1) / best_c + 1) / 2 * 24;  // an even number of blocks (TMA store pairs)
+  const uint64_t len = ((blocks + best_c - 1) / best_c + 7) / 8 * 96;  // whole cycles of 8 blocks (StreamMajorStage)
   *chunk_len = len;
   *n_chunks = (uint32_t)((n_per + len - 1) / len);
 }
@@ -957,7 +1006,8 @@ static unsigned tc_slots() {
   return slots;
 }
 
-// Tensor map of a stream-major output (UMMA engine, aligned): out[count][n_per] doubles, box 32 x 24.
+// Tensor map of a stream-major output (UMMA engine, aligned): out[count][n_per] doubles viewed as
+// [count][n_per / 16][16], box 32 x 2 x 16, 128-byte swizzle (StreamMajorStage).  n_per >= 16.
 // cuTensorMapEncodeTiled comes from the driver through the runtime (no link against libcuda).
 static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count, uint64_t n_per) {
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -973,12 +1023,12 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
   }
   if (n_per >= (1ull << 31) || count >= (1ull << 31))
     return fail(RLXPP_EINVAL, "stream-major output: n_per_stream and the stream count must be below 2^31");
-  const cuuint64_t dims[2] = {n_per, count};
-  const cuuint64_t strides[1] = {n_per * sizeof(double)};
-  const cuuint32_t box[2] = {kStageBoxCols, 32};
-  const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, out, dims, strides, box, estr,
-                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+  const cuuint64_t dims[3] = {16, n_per / 16, count};
+  const cuuint64_t strides[2] = {16 * sizeof(double), n_per * sizeof(double)};
+  const cuuint32_t box[3] = {16, 2, 32};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, out, dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
   return RLXPP_OK;
@@ -986,7 +1036,7 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
 
 template <int MODE, int OUT = kF64>
 static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
-  if (MODE == kStoreStreamMajor && aligned) {
+  if (MODE == kStoreStreamMajor && aligned && a.n_per >= kStageCycle) {  // shorter rows never reach the TMA path
     const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per);
     if (rc) return rc;
   }
@@ -996,14 +1046,30 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len);
   if (g_force_chunks.load() > 0 && a.n_per / 12 >= (uint64_t)g_force_chunks.load()) {  // test hook
     const uint64_t c = (uint64_t)g_force_chunks.load(), blocks = a.n_per / 12;
-    a.chunk_len = ((blocks + c - 1) / c + 1) / 2 * 24;
+    a.chunk_len = ((blocks + c - 1) / c + 7) / 8 * 96;
     a.n_chunks = (u32)((a.n_per + a.chunk_len - 1) / a.chunk_len);
   }
   const uint64_t items = n_tiles * a.n_chunks;
   const unsigned grid = (unsigned)(items < slots ? items : slots);
   CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
-  if (aligned) tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, 0, s>>>(a);
-  else tc_generate_kernel<MODE, false, OUT><<<grid, tc::kTile, 0, s>>>(a);
+  if (aligned) {
+    constexpr bool kStaged = MODE == kStoreStreamMajor;  // the kernel's kStaged
+    if (kStaged) {  // 20 KB static + 33 KB of boxes: above the 48 KB default, 4 CTAs per SM still fit
+      static std::atomic<uint64_t> done{0};  // one bit per device: function attributes are per device
+      int dev = 0;
+      CUDA_TRY(cudaGetDevice(&dev));
+      if (dev >= 64 || !(done.load() >> dev & 1)) {
+        CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)kStageCtaBytes));
+        CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                      cudaSharedmemCarveoutMaxShared));
+        if (dev < 64) done.fetch_or(1ull << dev);
+      }
+    }
+    tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, kStaged ? kStageCtaBytes : 0, s>>>(a);
+  } else {
+    tc_generate_kernel<MODE, false, OUT><<<grid, tc::kTile, 0, s>>>(a);
+  }
   LAUNCH_CHECK();
   return RLXPP_OK;
 }
@@ -1515,6 +1581,39 @@ int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s,
     float ms = 0.f;
     CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
     const double rate = (double)(bytes / 16 * 16) / (ms * 1e-3);
+    if (it >= 2 && rate > best) best = rate;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(buf);
+  *bytes_per_s = best;
+  return RLXPP_OK;
+}
+
+int rlxpp_measure_hbm_write_pieces(uint64_t rows, uint64_t pitch_bytes, uint32_t piece_bytes, int iters, double* bytes_per_s,
+                                   void* cuda_stream) {
+  if (!bytes_per_s || iters <= 0 || rows < 32 || rows % 32 || piece_bytes < 16 || piece_bytes % 16 || pitch_bytes % 16 ||
+      pitch_bytes < piece_bytes)
+    return fail(RLXPP_EINVAL, "rlxpp_measure_hbm_write_pieces: rows must be a multiple of 32, piece and pitch multiples of 16 bytes");
+  int rc = check_device();
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  uint4* buf = nullptr;
+  CUDA_TRY(cudaMalloc(&buf, rows * pitch_bytes));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  const uint64_t written = rows * (pitch_bytes / piece_bytes) * piece_bytes;
+  double best = 0.0;
+  for (int it = 0; it < iters + 2; it++) {
+    CUDA_TRY(cudaEventRecord(e0, s));
+    hbm_write_pieces_kernel<<<tc_slots(), 128, 0, s>>>(buf, rows, pitch_bytes / 16, piece_bytes / 16);
+    g_launches++;
+    CUDA_TRY(cudaEventRecord(e1, s));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    const double rate = (double)written / (ms * 1e-3);
     if (it >= 2 && rate > best) best = rate;
   }
   cudaEventDestroy(e0);

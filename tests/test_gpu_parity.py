@@ -158,21 +158,27 @@ def test_cfg3_interleaved_small(rlx, torch, oracle, nthreads):
     check_state(rlx, torch, h, ref, "cfg3 small")
 
 
-def test_cfg3_full_size_sampled(rlx, torch, oracle, nthreads):
+@pytest.mark.parametrize("layout", ["interleaved", "stream_major"])
+def test_cfg3_full_size_sampled(rlx, torch, oracle, nthreads, layout):
     """BASELINE.json configs[2] in bench.py's launch configuration: 2^20 streams x 1,536 doubles,
-    interleaved, 12.9 GB.  Sampled streams (first and last blocks, a stride through the rest) are
-    compared in full; the whole array is checked for range and lattice on the device."""
+    12.9 GB, interleaved (the config's layout) and stream-major (bench.py --layout stream_major).  Sampled
+    streams (first and last blocks, a stride through the rest) are compared in full; the whole array is
+    checked for range and lattice on the device."""
     n, per = 1 << 20, 1536
     h = rlx.rlxpp_create(n, 1, 2048)
-    out = torch.empty((per, n), dtype=torch.float64, device="cuda")
-    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+    il = layout == "interleaved"
+    out = torch.empty((per, n) if il else (n, per), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED if il else rlx.RLXPP_STREAM_MAJOR)
     torch.cuda.synchronize()
     idx = np.unique(np.concatenate([np.arange(0, 130), np.arange(n - 130, n), np.arange(0, n, 4099)]))
-    got = out[:, torch.from_numpy(idx).cuda()].cpu().numpy().T
+    tidx = torch.from_numpy(idx).cuda()
+    got = out[:, tidx].cpu().numpy().T if il else out[tidx].cpu().numpy()
     ref = oracle.streams(inputs.seeds(n)[idx], 2048, per, want=("doubles", "state"), nthreads=nthreads)
-    assert_bits_equal(got, ref["doubles"], "cfg3 full (sampled streams)")
-    for lo in range(0, per, 128):  # properties at any size, chunked to bound temporaries
-        blk = out[lo:lo + 128]
+    assert_bits_equal(got, ref["doubles"], f"cfg3 full, {layout} (sampled streams)")
+    flat = out.view(-1)
+    step = 128 * n
+    for lo in range(0, per * n, step):  # properties at any size, chunked to bound temporaries
+        blk = flat[lo:lo + step]
         assert bool((blk >= 0).all()) and bool((blk < 1).all())
         sc = blk * 2.0**48
         assert bool((sc == sc.floor()).all())
@@ -505,6 +511,29 @@ def test_chunked_work_items_give_the_same_results(rlx, torch, oracle, nthreads, 
         rlx.rlxpp_destroy(h)
     finally:
         rlx.rlxpp_set_chunks(0)
+
+
+@pytest.mark.parametrize("blocks", [1, 7, 8, 9, 15, 16, 21, 43])
+def test_stream_major_rows_of_any_length(rlx, torch, oracle, nthreads, blocks):
+    """Stream-major output, aligned cursors (UMMA engine: 256-byte boxes through the TMA for whole cycles of
+    8 blocks, direct stores for the rest of a row; rlxpp.cu StreamMajorStage).  Row lengths on both sides of
+    the cycle, rows that are not 128- or 256-byte multiples, a ragged last warp and tile (rows the tensor
+    map must clip), and a guard band behind the buffer that must stay untouched.  Two calls in a row: the
+    second continues the streams."""
+    n, per = 3 * 128 + 45, 12 * blocks
+    guard = 4096
+    h = rlx.rlxpp_create(n, 77, 2048)
+    ref = oracle.streams(inputs.seeds(n, 77), 2048, 2 * per, want=("doubles", "state"), nthreads=nthreads)
+    for call in range(2):
+        buf = torch.full((n * per + guard,), -1.0, dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_doubles(h, buf, per, rlx.RLXPP_STREAM_MAJOR)
+        torch.cuda.synchronize()
+        got = buf.cpu().numpy()
+        assert_bits_equal(got[:n * per].reshape(n, per), ref["doubles"][:, call * per:(call + 1) * per],
+                          f"stream-major rows of {blocks} blocks, call {call}")
+        assert np.all(got[n * per:] == -1.0), "wrote behind the output buffer"
+    check_state(rlx, torch, h, ref, "stream-major rows")
+    rlx.rlxpp_destroy(h)
 
 
 def test_generic_multiplier_streams(rlx, torch, oracle, nthreads):
