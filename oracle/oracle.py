@@ -167,3 +167,12 @@ def engine_run(X: int, pos: int, p: int, ops):
     _lib.orc_engine_run(_p(x, _u64p), ctypes.byref(pp), ctypes.c_uint32(p), _p(is_skip, _u8p), _p(amount, _u64p),
                         ctypes.c_int(len(ops)), _p(out, _u64p))
     return limbs_to_int(x), int(pp.value), [int(v) for v in out[:ndraw]]
+
+
+def normals(k48) -> np.ndarray:
+    """Box-Muller normals of consecutive PAIRS of 48-bit draws along the last axis (even length)."""
+    k = np.ascontiguousarray(k48, dtype=np.uint64)
+    assert k.shape[-1] % 2 == 0
+    z = np.zeros(k.shape, np.float64)
+    _lib.orc_normals(_p(k, _u64p), ctypes.c_uint64(k.size // 2), _p(z, _f64p))
+    return z

@@ -23,6 +23,9 @@
 //   * swb_step / to_lcg / to_ranlux / advance              : pinned (advance by
 //     a^p == p direct subtract-with-borrow steps; closed form == long division
 //     == digit formula; tiny-parameter exhaustive check of the state map).
+//   * normals (SURVEY 8f-2 "a distribution on top (Gaussian)"; the paper names no
+//     transform: reading N-1 in DESIGN.md, Box-Muller)   : pinned (Python math
+//     functions; z0^2 + z1^2 and atan2(z1, z0); special arguments; sample moments).
 //   * draw order / bit order inside uint64[9] (S8c-5), "advance first" (S8c-6),
 //     seeding exponent 2^96 (S8c-7): conventions, PARITY UNPINNED against
 //     ROOT's RanluxppEngine (no values are printed in the paper).
@@ -493,6 +496,38 @@ void orc_engine_run(u64* X9, unsigned* pos, uint32_t p, const unsigned char* is_
   }
   memcpy(X9, e.X, sizeof(e.X));
   *pos = (unsigned)e.pos;
+}
+
+// Standard normal deviates from pairs of 48-bit draws (reading N-1; not in the paper, which
+// stops at uniform numbers).  The plain Box-Muller definition (Box & Muller 1958) on
+// u0 = k[2i] 2^-48, u1 = k[2i+1] 2^-48, both in [0, 1):
+//     r = sqrt(-2 ln(1 - u0)),   z[2i] = r cos(2 pi u1),   z[2i+1] = r sin(2 pi u1)
+// (1 - u0 is in (0, 1] and exact, so the logarithm is finite).  Evaluated in long double (x87 64-bit
+// mantissa) and rounded once to fp64.  cos / sin of 2 pi u1 use the exact identities for a quarter
+// turn and its complement -- t = 4 u1 is exact, q = floor(t), f = t - q, angle = (pi / 2) f, and
+// cos(pi/2 f) = sin(pi/2 (1 - f)) for f > 1/2 -- so that the exact zeros of the definition
+// (u1 = 0, 1/4, 1/2, 3/4) are zeros here too and the relative error is ~2^-63 everywhere, also next to them.
+void orc_normals(const u64* k, u64 n_pairs, double* z) {
+  const long double half_pi = 1.57079632679489661923132169163975144L;
+  for (u64 i = 0; i < n_pairs; i++) {
+    const double u0 = (double)k[2 * i] * 0x1p-48, u1 = (double)k[2 * i + 1] * 0x1p-48;
+    const long double r = sqrtl(-2.0L * logl(1.0L - (long double)u0));
+    const double t = 4.0 * u1;                 // exact
+    const int q = (int)t;                      // 0 .. 3
+    const double f = t - (double)q;            // exact, in [0, 1)
+    const bool upper = f > 0.5;                // cos(pi/2 f) = sin(pi/2 (1 - f)): arguments stay in [0, pi/4]
+    const long double ang = half_pi * (long double)(upper ? 1.0 - f : f);
+    const long double c = upper ? sinl(ang) : cosl(ang), s = upper ? cosl(ang) : sinl(ang);
+    long double cq, sq;                        // cos, sin of ang + q pi / 2
+    switch (q) {
+      case 0: cq = c; sq = s; break;
+      case 1: cq = -s; sq = c; break;
+      case 2: cq = -c; sq = -s; break;
+      default: cq = s; sq = -c; break;
+    }
+    z[2 * i] = (double)(r * cq);
+    z[2 * i + 1] = (double)(r * sq);
+  }
 }
 
 int orc_hardware_threads(void) {

@@ -464,3 +464,100 @@ def test_splitmix64_and_cfg2_inputs(oracle):
     A16 = pow(A1, 2048 * 16, M)
     for i in list(range(0, 256, 17)) + list(range(256, 320)):
         assert inputs.limbs_to_int(out[i]) == A16 * inputs.limbs_to_int(st[i]) % M
+
+
+# ----------------------------------------------------------------- normals (DESIGN reading N-1)
+def _dec_pi_sin_cos(prec=60):
+    """pi, sin, cos in `decimal` at `prec` digits (Machin's formula and Taylor series): the independent side."""
+    import decimal
+    D = decimal.Decimal
+    ctx = decimal.Context(prec=prec)
+
+    def atan_inv(n):  # atan(1 / n)
+        x, total, k, n2 = D(1) / D(n), D(0), 0, D(n) * D(n)
+        with decimal.localcontext(ctx):
+            term = D(1) / D(n)
+            while abs(term) > D(10) ** (-prec - 5):
+                total += term / (2 * k + 1) if k % 2 == 0 else -term / (2 * k + 1)
+                term /= n2
+                k += 1
+        return total
+
+    with decimal.localcontext(ctx):
+        pi = 16 * atan_inv(5) - 4 * atan_inv(239)
+
+    def sincos(x):
+        with decimal.localcontext(ctx):
+            s, c, term, k = D(0), D(0), D(1), 0
+            while abs(term) > D(10) ** (-prec - 5):
+                if k % 2 == 0:
+                    c += term if (k // 2) % 2 == 0 else -term
+                else:
+                    s += term if (k // 2) % 2 == 0 else -term
+                k += 1
+                term = term * x / k
+            return s, c
+
+    return ctx, pi, sincos
+
+
+def test_normals_are_box_muller_to_the_last_bit_or_so(oracle):
+    """orc_normals against 60-digit decimal arithmetic (ln and sqrt from `decimal`, pi / sin / cos above): the fp64
+    result is within 1 ulp of the exact Box-Muller value, including arguments next to the zeros of sin and cos."""
+    import decimal
+    D = decimal.Decimal
+    ctx, pi, sincos = _dec_pi_sin_cos()
+    rng = random.Random(48)
+    quarter = 1 << 46
+    ks = [(rng.randrange(1 << 48), rng.randrange(1 << 48)) for _ in range(40)]
+    ks += [(rng.randrange(1 << 48), q * quarter + d) for q in range(4) for d in (1, 2, 12345)]
+    ks += [(rng.randrange(1 << 48), (q * quarter - d) % (1 << 48)) for q in range(4) for d in (1, 777)]
+    ks += [(1, 5), ((1 << 48) - 1, 99), (1 << 47, 1 << 45)]
+    z = oracle.normals(np.array(ks, dtype=np.uint64).reshape(-1))
+    for i, (k0, k1) in enumerate(ks):
+        with decimal.localcontext(ctx):
+            u0, u1 = D(k0) / D(1 << 48), D(k1) / D(1 << 48)
+            r = (-2 * (1 - u0).ln()).sqrt()
+            s, c = sincos(2 * pi * u1)
+            want = (r * c, r * s)
+        for got, w in zip(z[2 * i:2 * i + 2], want):
+            assert abs(D(float(got)) - w) <= D(float(np.spacing(abs(got)))), (k0, k1, got, w)
+
+
+def test_normals_pairing_special_arguments_and_python_math(oracle):
+    import math
+    rng = random.Random(7)
+    ks = [(rng.randrange(1 << 48), rng.randrange(1 << 48)) for _ in range(2000)]
+    z = oracle.normals(np.array(ks, dtype=np.uint64).reshape(-1)).reshape(-1, 2)
+    for (k0, k1), (z0, z1) in zip(ks, z):
+        u0, u1 = k0 / 2**48, k1 / 2**48
+        r2 = -2.0 * math.log(1.0 - u0)
+        r = math.sqrt(r2)
+        # the first draw of a pair sets the radius, the second the angle; cos first, sin second
+        assert math.isclose(z0 * z0 + z1 * z1, r2, rel_tol=1e-14)
+        dphi = (math.atan2(z1, z0) - 2 * math.pi * u1) % (2 * math.pi)
+        assert min(dphi, 2 * math.pi - dphi) < 1e-14
+        assert abs(z0 - r * math.cos(2 * math.pi * u1)) <= 4e-15 * max(r, 1.0)
+        assert abs(z1 - r * math.sin(2 * math.pi * u1)) <= 4e-15 * max(r, 1.0)
+    # exact zeros of the definition; u0 = 0 gives r = 0; the largest radius is sqrt(2 * 48 ln 2)
+    k0 = 123456789 << 10
+    r = math.sqrt(-2.0 * math.log(1.0 - k0 / 2**48))
+    sp = oracle.normals(np.array([k0, 0, k0, 1 << 46, k0, 1 << 47, k0, 3 << 46, 0, 12345, (1 << 48) - 1, 0], dtype=np.uint64))
+    assert list(sp[:8]) == [r, 0.0, 0.0, r, -r, 0.0, 0.0, -r]
+    assert sp[8] == 0.0 and sp[9] == 0.0
+    assert math.isclose(sp[10], math.sqrt(96 * math.log(2)), rel_tol=1e-15) and sp[11] == 0.0
+
+
+def test_normals_are_standard_normal_in_distribution(oracle):
+    """Sample moments of 4 x 10^5 deviates made from a RANLUX++ stream (5 sigma bands of the sampling error)."""
+    n = 400_000
+    k = oracle.streams(inputs.seeds(1, 2024), 2048, n, want=("ints",))["ints"].reshape(-1)
+    z = oracle.normals(k)
+    se = 1.0 / np.sqrt(n)
+    assert abs(z.mean()) < 5 * se
+    assert abs(z.var() - 1.0) < 5 * np.sqrt(2.0) * se
+    assert abs((z**3).mean()) < 5 * np.sqrt(15.0) * se
+    assert abs((z**4).mean() - 3.0) < 5 * np.sqrt(96.0) * se
+    p1 = 0.6826894921370859  # P(|Z| < 1)
+    assert abs((np.abs(z) < 1.0).mean() - p1) < 5 * np.sqrt(p1 * (1 - p1)) * se
+    assert abs(np.mean(z[0::2] * z[1::2])) < 5 * np.sqrt(2.0) * se  # the two halves of a pair are uncorrelated
