@@ -194,9 +194,10 @@ def main():
                     help="luxury level (default: the workload's, 2048); BASELINE configs[3] sweeps 24, 389, 1024, 2048")
     ap.add_argument("--layout", default="interleaved", choices=["interleaved", "stream_major"],
                     help="cfg3 / cfg4 output layout (BASELINE cfg3 names the interleaved one; stream_major is context)")
-    ap.add_argument("--output", default="f64", choices=["f64", "u48", "f32"],
+    ap.add_argument("--output", default="f64", choices=["f64", "u48", "f32", "normal"],
                     help="cfg3 / cfg4: what a 48-bit draw is stored as (SURVEY 8f-2): the double (BASELINE), the integer, "
-                         "or its two 24-bit floats; `value` stays in 48-bit draws per second")
+                         "its two 24-bit floats, or a standard normal deviate (Box-Muller, fused); `value` stays in "
+                         "48-bit draws per second")
     ap.add_argument("--chunks", type=int, default=0,
                     help="UMMA engine: force the number of chunks per tile (rlxpp_set_chunks; 0 = the library decides)")
     ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
@@ -259,6 +260,8 @@ def main():
                 rlx.rlxpp_generate_u48(h, out, n_per, lay)
             elif args.output == "f32":
                 rlx.rlxpp_generate_floats(h, out, 2 * n_per, lay)
+            elif args.output == "normal":
+                rlx.rlxpp_generate_normal(h, out, n_per, lay)
             else:
                 rlx.rlxpp_generate_doubles(h, out, n_per, lay)
     elif args.workload == "cfg5":

@@ -145,6 +145,16 @@ int rlxpp_set_chunks(int n_chunks);
  * rlxpp_generate_doubles, plus EINVAL for an odd float count. */
 int rlxpp_generate_u48(rlxpp_t* h, uint64_t* out_dev, uint64_t n_per_stream, int layout);
 int rlxpp_generate_floats(rlxpp_t* h, float* out_dev, uint64_t n_per_stream, int layout);
+/* rlxpp_generate_normal: standard normal deviates, fused into the generation kernel (SURVEY 8f-2 "a distribution
+ *   on top (Gaussian)"; the paper stops at uniform numbers, so the transform is this
+ *   library's: DESIGN.md reading N-1).  Box-Muller on the stream's draw pairs (2i, 2i + 1), counted from the
+ *   stream's first draw: u0 = k[2i] 2^-48, u1 = k[2i+1] 2^-48, r = sqrt(-2 ln(1 - u0)); the deviate at draw
+ *   position 2i is r cos(2 pi u1), at 2i + 1 r sin(2 pi u1).  One deviate per draw position: the call consumes
+ *   n_per_stream draws of every stream, any cursor, any count, and interleaves freely with the other generate
+ *   calls and with skips (a call that starts or ends inside a pair evaluates that pair twice).  fp64
+ *   log / sqrt / sincospi: within 6 ulp of the exact value (the only output form that is not bit-exact);
+ *   |z| <= sqrt(96 ln 2) = 8.157.  Layouts, ownership and errors as rlxpp_generate_doubles; UMMA engine. */
+int rlxpp_generate_normal(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout);
 
 /* ---- Host engine ------------------------------------------
  * ONE stream continued on the host, with the library's own host arithmetic: the same sequence as the

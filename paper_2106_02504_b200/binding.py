@@ -53,6 +53,7 @@ _SIGNATURES = {
     "rlxpp_set_chunks": (ctypes.c_int, [ctypes.c_int]),
     "rlxpp_generate_u48": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
     "rlxpp_generate_floats": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
+    "rlxpp_generate_normal": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
     "rlxpp_host_generate": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64,
                                            ctypes.c_uint64, ctypes.c_void_p]),
     "rlxpp_device_view": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
@@ -183,6 +184,10 @@ def rlxpp_generate_u48(h: Handle, out_dev, n_per_stream: int, layout: int = RLXP
 
 def rlxpp_generate_floats(h: Handle, out_dev, n_per_stream: int, layout: int = RLXPP_STREAM_MAJOR):
     _check(load().rlxpp_generate_floats(h.ptr, _ptr(out_dev), n_per_stream, layout), "rlxpp_generate_floats")
+
+
+def rlxpp_generate_normal(h: Handle, out_dev, n_per_stream: int, layout: int = RLXPP_STREAM_MAJOR):
+    _check(load().rlxpp_generate_normal(h.ptr, _ptr(out_dev), n_per_stream, layout), "rlxpp_generate_normal")
 
 
 def rlxpp_host_generate(lcg: np.ndarray, pos: int, p: int, skip: int, n: int):

@@ -257,8 +257,7 @@ struct GenArgs {
   u32 n_tiles, n_chunks;
   u64 chunk_len;      // draws per chunk (a multiple of 12 when n_chunks > 1)
   u32 kexp = kExp16;  // see arith.cuh: a launch parameter on purpose
-  // UMMA engine, aligned stream-major stores: tensor map of out as [count streams][n_per] doubles,
-  // box = 32 streams x 24 doubles
+  // UMMA engine, aligned stream-major stores: tensor map of out (StreamMajorStage)
   alignas(64) CUtensorMap tmap;
 };
 
@@ -266,7 +265,9 @@ enum { kStoreStreamMajor = 0, kStoreInterleaved = 1, kReduce = 2 };
 // What a 48-bit draw is written as (S8 f-2): the double k 2^-48; the integer k as uint64; or its two
 // 24-bit RANLUX numbers as floats x 2^-24 (low number first).  Every form is 8 bytes per draw, carried
 // through the emission code as the bit pattern of a double.
-enum { kF64 = 0, kU48 = 1, kF32 = 2 };
+// kNormal (reading N-1 in DESIGN.md): a standard normal deviate per draw position, Box-Muller on the draw pair
+// (2i, 2i + 1) of the block -- fp64 log / sqrt / sincospi, the only output form that is not exact (<= 6 ulp).
+enum { kF64 = 0, kU48 = 1, kF32 = 2, kNormal = 3 };
 
 template <int OUT, int J>
 __device__ __forceinline__ double draw_value(const u32 (&v)[18], u32 kexp) {
@@ -283,6 +284,23 @@ __device__ __forceinline__ double draw_value(const u32 (&v)[18], u32 kexp) {
   const float f0 = __uint2float_rn(lo & 0xFFFFFFu) * 0x1p-24f;               // RANLUX number 2J (exact)
   const float f1 = __uint2float_rn(__byte_perm(lo, hi, 0x6543)) * 0x1p-24f;  // number 2J + 1 = bits 24..47
   return __hiloint2double(__float_as_int(f1), __float_as_int(f0));
+}
+
+// draws J (even) and J + 1 of the block in output form OUT
+template <int OUT, int J>
+__device__ __forceinline__ void draw_pair(const u32 (&v)[18], u32 kexp, double& a, double& b) {
+  static_assert(J % 2 == 0, "pairs start at even draws");
+  if constexpr (OUT == kNormal) {
+    const double u0 = draw_double<J>(v, kexp), u1 = draw_double<J + 1>(v, kexp);
+    const double r = sqrt(-2.0 * log(1.0 - u0));  // 1 - u0 is exact and in (0, 1]
+    double sn, cs;
+    sincospi(2.0 * u1, &sn, &cs);                 // exact argument: no 2 pi rounding, exact zeros
+    a = r * cs;
+    b = r * sn;
+  } else {
+    a = draw_value<OUT, J>(v, kexp);
+    b = draw_value<OUT, J + 1>(v, kexp);
+  }
 }
 
 template <int MODE, int OUT = kF64>
@@ -307,10 +325,18 @@ struct EmitBlock {
   // all 12 draws of block v go to output indices t0 .. t0 + 11 (VEC: t0 is even and p is 16-byte aligned)
   template <bool VEC = true>
   static __device__ __forceinline__ void all(Sink<MODE, OUT>& s, const u32 (&v)[18], u64 t0) {
-    if (MODE == kStoreStreamMajor && VEC) {
-      if (J % 2 == 0) {  // two draws per 128-bit store (p + t0 is 16-byte aligned: n_per % 12 == 0)
-        double2 d2 = make_double2(draw_value<OUT, J>(v, s.kexp), draw_value<OUT, J + 1>(v, s.kexp));
+    if constexpr (MODE == kStoreStreamMajor && VEC) {
+      if constexpr (J % 2 == 0) {  // two draws per 128-bit store (p + t0 is 16-byte aligned: n_per % 12 == 0)
+        double2 d2;
+        draw_pair<OUT, J>(v, s.kexp, d2.x, d2.y);
         __stcs(reinterpret_cast<double2*>(s.p + t0 + J), d2);
+      }
+    } else if constexpr (OUT == kNormal) {
+      if constexpr (J % 2 == 0) {
+        double a, b;
+        draw_pair<OUT, J>(v, s.kexp, a, b);
+        s.emit(t0 + J, a);
+        s.emit(t0 + J + 1, b);
       }
     } else {
       s.emit(t0 + J, draw_value<OUT, J>(v, s.kexp));
@@ -320,10 +346,21 @@ struct EmitBlock {
   // draw J of the block at absolute draw position q0 + J is output index q0 + J - pos if in [0, n)
   static __device__ __forceinline__ void masked(Sink<MODE, OUT>& s, const u32 (&v)[18], u64 q0, u32 pos, u64 n) {
     const u64 t = q0 + J - pos;  // wraps when q0 + J < pos: then t >= n
-    const bool valid = t < n;
-    const double d = draw_value<OUT, J>(v, s.kexp);
-    if (MODE == kReduce) s.emit(t, valid ? d : 0.0);  // + 0.0 and fma(0, 0, Q) are exact no-ops
-    else if (valid) s.emit(t, d);
+    if constexpr (OUT == kNormal) {
+      if constexpr (J % 2 == 0) {  // the deviate of a draw position depends on both draws of its pair
+        if (t < n || t + 1 < n) {
+          double a, b;
+          draw_pair<OUT, J>(v, s.kexp, a, b);
+          if (t < n) s.emit(t, a);
+          if (t + 1 < n) s.emit(t + 1, b);
+        }
+      }
+    } else {
+      const bool valid = t < n;
+      const double d = draw_value<OUT, J>(v, s.kexp);
+      if (MODE == kReduce) s.emit(t, valid ? d : 0.0);  // + 0.0 and fma(0, 0, Q) are exact no-ops
+      else if (valid) s.emit(t, d);
+    }
     EmitBlock<J + 1, MODE, OUT>::masked(s, v, q0, pos, n);
   }
 };
@@ -420,6 +457,7 @@ struct StreamMajorStage {
   const void* tmap;
   u32 kexp;       // exp16()
   u32 cv[18];     // limbs of the block whose last draws wait for the next box (only [6, 18) are ever live)
+  double cz[8];   // kNormal: the waiting deviates themselves
   __device__ __forceinline__ void init(uint8_t* stage, const void* tensor_map, u64 tile_first, u32 kexp_, u64 t0) {
     const u32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     box = ((umma::smem_u32(stage) + 1023u) & ~1023u) + warp * kStageWarpBytes;
@@ -436,8 +474,19 @@ struct StreamMajorStage {
   template <int OUT, int J, int O>
   __device__ __forceinline__ void put2(const u32 (&v)[18]) {
     constexpr u32 h = (u32)O >> 7, K = ((((u32)O >> 4) & 7u) ^ h) << 4;
-    const double a = draw_value<OUT, J>(v, kexp), b = draw_value<OUT, J + 1>(v, kexp);
+    double a, b;
+    draw_pair<OUT, J>(v, kexp, a, b);
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"((rowbase | (rs ^ K)) + h * 128u), "d"(a), "d"(b) : "memory");
+  }
+  // doubles z[J0 .. J1) to byte offset O of the lane's row
+  template <int J0, int J1, int O>
+  __device__ __forceinline__ void putd(const double* z) {
+    if constexpr (J0 < J1) {
+      constexpr u32 h = (u32)O >> 7, K = ((((u32)O >> 4) & 7u) ^ h) << 4;
+      asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"((rowbase | (rs ^ K)) + h * 128u), "d"(z[J0]), "d"(z[J0 + 1])
+                   : "memory");
+      putd<J0 + 2, J1, O + 16>(z);
+    }
   }
   template <int OUT, int J0, int J1, int O>
   struct Put {
@@ -469,6 +518,34 @@ struct StreamMajorStage {
   // whole-warp call: the next block of the item (blocks come in whole cycles of 8)
   template <int OUT>
   __device__ __forceinline__ void emit(const u32 (&v)[18]) {
+    if constexpr (OUT == kNormal) {
+      // the transform is too long to sit in all eight phases (instruction cache): evaluate the block first, then
+      // place it; straddling deviates are carried as doubles (cz[j - 4] = z[j])
+      double z[12];
+      draw_pair<OUT, 0>(v, kexp, z[0], z[1]);
+      draw_pair<OUT, 2>(v, kexp, z[2], z[3]);
+      draw_pair<OUT, 4>(v, kexp, z[4], z[5]);
+      draw_pair<OUT, 6>(v, kexp, z[6], z[7]);
+      draw_pair<OUT, 8>(v, kexp, z[8], z[9]);
+      draw_pair<OUT, 10>(v, kexp, z[10], z[11]);
+      switch (q) {
+        case 0: wait_box(); putd<0, 12, 0>(z); break;
+        case 1: putd<0, 12, 96>(z); break;
+        case 2: putd<0, 8, 192>(z); send(); cz[4] = z[8]; cz[5] = z[9]; cz[6] = z[10]; cz[7] = z[11]; break;
+        case 3: wait_box(); putd<4, 8, 0>(cz); putd<0, 12, 32>(z); break;
+        case 4: putd<0, 12, 128>(z); break;
+        case 5:
+          putd<0, 4, 224>(z);
+          send();
+#pragma unroll
+          for (int j = 0; j < 8; j++) cz[j] = z[j + 4];
+          break;
+        case 6: wait_box(); putd<0, 8, 0>(cz); putd<0, 12, 64>(z); break;
+        default: putd<0, 12, 160>(z); send(); break;
+      }
+      q = (q + 1u) & 7u;
+      return;
+    }
     switch (q) {
       case 0: wait_box(); Put<OUT, 0, 12, 0>::all(*this, v); break;
       case 1: Put<OUT, 0, 12, 96>::all(*this, v); break;
@@ -1335,6 +1412,9 @@ static int generate_other(rlxpp_t* h, void* out_dev, uint64_t n_draws, int layou
   if (kind == kU48)
     rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor, kU48>(a, aligned, h->stream)
                                       : launch_tc_generate_mode<kStoreInterleaved, kU48>(a, aligned, h->stream);
+  else if (kind == kNormal)
+    rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor, kNormal>(a, aligned, h->stream)
+                                      : launch_tc_generate_mode<kStoreInterleaved, kNormal>(a, aligned, h->stream);
   else
     rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor, kF32>(a, aligned, h->stream)
                                       : launch_tc_generate_mode<kStoreInterleaved, kF32>(a, aligned, h->stream);
@@ -1350,6 +1430,10 @@ int rlxpp_generate_u48(rlxpp_t* h, uint64_t* out_dev, uint64_t n_per_stream, int
 int rlxpp_generate_floats(rlxpp_t* h, float* out_dev, uint64_t n_per_stream, int layout) {
   if (n_per_stream % 2) return fail(RLXPP_EINVAL, "rlxpp_generate_floats: n_per_stream must be even (two floats per 48-bit draw)");
   return generate_other(h, out_dev, n_per_stream / 2, layout, kF32, "rlxpp_generate_floats");
+}
+
+int rlxpp_generate_normal(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout) {
+  return generate_other(h, out_dev, n_per_stream, layout, kNormal, "rlxpp_generate_normal");
 }
 
 static int ensure_staging(rlxpp_t* h, size_t bytes_each) {

@@ -315,6 +315,59 @@ def test_u48_and_float_outputs_are_the_same_draws(rlx, torch, oracle, nthreads, 
     rlx.rlxpp_destroy(h)
 
 
+NORMAL_ULPS = 6  # log <= 1 ulp (halved by the sqrt), sqrt and product 0.5 each, sincospi <= 2, oracle 0.5
+
+
+def assert_within_ulps(got, want, ulps, what):
+    got, want = np.asarray(got), np.asarray(want)
+    assert got.shape == want.shape, (what, got.shape, want.shape)
+    bad = np.nonzero(~(np.abs(got - want) <= ulps * np.spacing(np.abs(want))))
+    assert bad[0].size == 0, f"{what}: {bad[0].size} values off by more than {ulps} ulp, first at " \
+                             f"{[int(b[0]) for b in bad]}: got {got[tuple(b[0] for b in bad)]!r} " \
+                             f"want {want[tuple(b[0] for b in bad)]!r}"
+
+
+@pytest.mark.parametrize("layout", ["stream_major", "interleaved"])
+def test_normal_deviates_are_box_muller_of_the_draw_pairs(rlx, torch, oracle, nthreads, layout):
+    """rlxpp_generate_normal (DESIGN reading N-1) against oracle.normals of the oracle's own 48-bit
+    draws.  One deviate per draw position: an aligned call (TMA boxes + directly stored tail when stream-major),
+    a call that ends inside a pair, one that starts inside a pair, and one after per-stream skips of random
+    parity; the cursor and state must be those of the same number of plain draws."""
+    n = 3 * 128 + 45
+    sm = layout == "stream_major"
+    lay = rlx.RLXPP_STREAM_MAJOR if sm else rlx.RLXPP_INTERLEAVED
+    dist = inputs.splitmix64(99, n) % np.uint64(1000)
+    counts = [12 * 19, 37, 41]
+    total = 12 * 19 + 37 + 41 + 1000 + 100
+    total += total % 2
+    k = oracle.streams(inputs.seeds(n, 5), 2048, total, want=("ints",), nthreads=nthreads)["ints"]
+    z = oracle.normals(k)  # pairs (2i, 2i + 1) counted from each stream's first draw
+    h = rlx.rlxpp_create(n, 5, 2048)
+
+    def call(per):
+        out = torch.full((n, per) if sm else (per, n), np.nan, dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_normal(h, out, per, lay)
+        torch.cuda.synchronize()
+        return out.cpu().numpy() if sm else out.cpu().numpy().T
+
+    at = 0
+    for per in counts:
+        assert_within_ulps(call(per), z[:, at:at + per], NORMAL_ULPS, f"normals {layout}, draws {at}..{at + per}")
+        at += per
+    rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    got = call(100)
+    want = np.stack([z[i, at + int(dist[i]):at + int(dist[i]) + 100] for i in range(n)])
+    assert_within_ulps(got, want, NORMAL_ULPS, f"normals {layout} after per-stream skips")
+    ref = oracle.streams(inputs.seeds(n, 5), 2048, 100, skips=dist + np.uint64(at), want=("state",), nthreads=nthreads)
+    check_state(rlx, torch, h, ref, "after normals")
+    # uniform doubles continue where the normals stopped
+    d = torch.empty((n, 24), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(h, d, 24, rlx.RLXPP_STREAM_MAJOR)
+    ref = oracle.streams(inputs.seeds(n, 5), 2048, 24, skips=dist + np.uint64(at + 100), want=("doubles",), nthreads=nthreads)
+    assert_bits_equal(d.cpu().numpy(), ref["doubles"], "doubles after normals")
+    rlx.rlxpp_destroy(h)
+
+
 def test_p24_floats_are_the_raw_ranlux_numbers(rlx, torch, oracle):
     """p = 24: the floats are the subtract-with-borrow numbers themselves (x 2^-24), one by one, from
     the oracle's direct SWB stepper (reading c-13)."""
