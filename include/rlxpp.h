@@ -113,6 +113,11 @@ int rlxpp_get_state(rlxpp_t* h, uint64_t* ranlux_dev, uint32_t* carry_dev, uint3
  * lcg_dev [n_streams][9] canonical LCG states (values >= m are reduced), pos_dev
  * [n_streams] cursors in [0, 12] (NULL = all 12).  Errors: EINVAL. */
 int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev);
+/* The same from the paper's stored form (SURVEY 8a-2 / reading D3 `to_lcg`): ranlux_dev
+ * [n_streams][9] = the 24 RANLUX numbers of 24 bits, oldest lowest, carry_dev [n_streams] in {0, 1} (NULL = all
+ * 0), as rlxpp_get_state exports them.  X = V - (V >> 336) + c on the device (V = 2^576 - 1 with c = 1 gives m,
+ * stored as 0).  pos_dev as above.  Errors: EINVAL. */
+int rlxpp_set_state_ranlux(rlxpp_t* h, const uint64_t* ranlux_dev, const uint32_t* carry_dev, const uint32_t* pos_dev);
 
 /* Host-only helpers: A = a^p mod m as computed by the library's own host arithmetic,
  * and the seed state (A^(2^96))^seed mod m.  out: 9 uint64_t on the host. */

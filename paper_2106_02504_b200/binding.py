@@ -45,6 +45,7 @@ _SIGNATURES = {
     "rlxpp_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                        ctypes.c_void_p]),
     "rlxpp_set_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "rlxpp_set_state_ranlux": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
     "rlxpp_multiplier": (ctypes.c_int, [ctypes.c_uint32, ctypes.c_void_p]),
     "rlxpp_seed_state": (ctypes.c_int, [ctypes.c_uint64, ctypes.c_uint32, ctypes.c_void_p]),
     "rlxpp_umma_matrix": (ctypes.c_int, [ctypes.c_uint32, ctypes.c_void_p]),
@@ -238,6 +239,10 @@ def rlxpp_get_state(h: Handle, ranlux_dev=None, carry_dev=None, pos_dev=None, lc
 
 def rlxpp_set_state(h: Handle, lcg_dev, pos_dev=None):
     _check(load().rlxpp_set_state(h.ptr, _ptr(lcg_dev), _ptr(pos_dev)), "rlxpp_set_state")
+
+
+def rlxpp_set_state_ranlux(h: Handle, ranlux_dev, carry_dev=None, pos_dev=None):
+    _check(load().rlxpp_set_state_ranlux(h.ptr, _ptr(ranlux_dev), _ptr(carry_dev), _ptr(pos_dev)), "rlxpp_set_state_ranlux")
 
 
 def rlxpp_multiplier(p: int) -> np.ndarray:

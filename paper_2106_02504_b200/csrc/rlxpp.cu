@@ -822,6 +822,45 @@ __global__ void __launch_bounds__(kThreads) import_kernel(uint4* __restrict__ st
   store_state(st, n, i, x, pos > 12u ? 12u : pos);
 }
 
+// S8 a-2 / D3: the paper's stored form -> LCG state, X = V - (V >> 336) + c, and X == m -> 0
+// (V = 2^576 - 1 with c = 1, the one combination that reaches m).  Cold path: the kernels keep the LCG form.
+__device__ __forceinline__ void to_lcg(const u32 (&v)[18], u32 c, u32 (&x)[18]) {
+  u32 z[20];
+  u64 borrow = 0;
+#pragma unroll
+  for (int j = 0; j < 18; j++) {
+    const u32 hi = j + 11 < 18 ? v[j + 11] : 0u, lo = j + 10 < 18 ? v[j + 10] : 0u;
+    const u64 d = (u64)v[j] - (u64)((lo >> 16) | (hi << 16)) - borrow;  // limb j of V >> 336
+    z[j] = (u32)d;
+    borrow = d >> 63;
+  }
+  u64 carry = c & 1u;
+#pragma unroll
+  for (int j = 0; j < 18; j++) {
+    const u64 t = (u64)z[j] + carry;
+    z[j] = (u32)t;
+    carry = t >> 32;
+  }
+  z[18] = 0; z[19] = 0;  // V >= V >> 336 and the sum is <= m: no borrow, no carry out
+  mod_m20(z, x);
+}
+
+__global__ void __launch_bounds__(kThreads) import_ranlux_kernel(uint4* __restrict__ st, u64 n, const u64* __restrict__ ranlux,
+                                                                 const u32* __restrict__ carry, const u32* __restrict__ pos_in) {
+  const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
+  if (i >= n) return;
+  u32 v[18], x[18];
+#pragma unroll
+  for (int l = 0; l < 9; l++) {
+    const u64 w = ranlux[i * 9 + l];
+    v[2 * l] = (u32)w;
+    v[2 * l + 1] = (u32)(w >> 32);
+  }
+  to_lcg(v, carry ? carry[i] : 0u, x);
+  u32 pos = pos_in ? pos_in[i] : 12u;
+  store_state(st, n, i, x, pos > 12u ? 12u : pos);
+}
+
 // ----------------------------------------------------------------------------- device API (S8 f-1)
 // rlxpp_generate_ragged[_reduce]: every stream draws ITS OWN number of doubles -- the paper's GPU use
 // (one state per thread, threads consume numbers at their own pace).  Written entirely
@@ -1522,6 +1561,16 @@ int rlxpp_get_state(rlxpp_t* h, uint64_t* ranlux_dev, uint32_t* carry_dev, uint3
 int rlxpp_set_state(rlxpp_t* h, const uint64_t* lcg_dev, const uint32_t* pos_dev) {
   if (!h || !lcg_dev) return fail(RLXPP_EINVAL, "rlxpp_set_state: null argument");
   import_kernel<<<grid_for(h->n), kThreads, 0, h->stream>>>(h->st, h->n, lcg_dev, pos_dev);
+  LAUNCH_CHECK();
+  h->pos_uniform = pos_dev == nullptr;
+  h->uniform_pos = 12;
+  h->aligned = h->pos_uniform;
+  return RLXPP_OK;
+}
+
+int rlxpp_set_state_ranlux(rlxpp_t* h, const uint64_t* ranlux_dev, const uint32_t* carry_dev, const uint32_t* pos_dev) {
+  if (!h || !ranlux_dev) return fail(RLXPP_EINVAL, "rlxpp_set_state_ranlux: null argument");
+  import_ranlux_kernel<<<grid_for(h->n), kThreads, 0, h->stream>>>(h->st, h->n, ranlux_dev, carry_dev, pos_dev);
   LAUNCH_CHECK();
   h->pos_uniform = pos_dev == nullptr;
   h->uniform_pos = 12;

@@ -632,6 +632,48 @@ def test_set_state_edge_states_and_roundtrip(rlx, torch, oracle):
 
 
 # ------------------------------------------------------------------------------------- host variants
+def test_set_state_from_the_papers_stored_form(rlx, torch, oracle, nthreads):
+    """SURVEY 8a-2 / reading D3: rlxpp_set_state_ranlux runs `to_lcg` (X = V - (V >> 336) + c) on the device.
+    (a) arbitrary packed numbers and both carries -- random, all zero, all ones (c = 1 reaches m -> 0), top ten
+    numbers all ones, only old / only new numbers -- against the oracle's to_lcg; (b) a generator moved through
+    get_state -> set_state_ranlux mid-block continues bit for bit."""
+    rng = np.random.default_rng(11)
+    full = (1 << 576) - 1
+    Vs = [0, 1, full, full, full - 1, full >> 240, (full >> 336) << 336, 1 << 336, (1 << 336) - 1, 1 << 575]
+    cs = [0, 1, 0, 1, 1, 1, 1, 0, 1, 0]
+    for _ in range(246):
+        Vs.append(int.from_bytes(rng.bytes(72), "little"))
+        cs.append(int(rng.integers(0, 2)))
+    n = len(Vs)
+    h = rlx.rlxpp_create(n, 1, 2048)
+    Vd = torch.from_numpy(np.stack([inputs.int_to_limbs(v) for v in Vs]).view(np.int64)).cuda()
+    cd = torch.from_numpy(np.array(cs, dtype=np.int32)).cuda()
+    rlx.rlxpp_set_state_ranlux(h, Vd, cd, None)
+    _, _, pos, X = gpu_state(rlx, torch, h)
+    for i in range(n):
+        assert inputs.limbs_to_int(X[i]) == oracle.to_lcg(Vs[i], cs[i]) % M, f"to_lcg case {i}"
+    assert np.all(pos == 12)
+    rlx.rlxpp_destroy(h)
+    # (b) hand-over in the stored form, cursors inside a block
+    n, first, rest = 300, 17, 43
+    a = rlx.rlxpp_create(n, 31, 2048)
+    d1 = torch.empty((n, first), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(a, d1, first, rlx.RLXPP_STREAM_MAJOR)
+    V = torch.empty((n, 9), dtype=torch.int64, device="cuda")
+    c = torch.empty(n, dtype=torch.int32, device="cuda")
+    pos = torch.empty(n, dtype=torch.int32, device="cuda")
+    rlx.rlxpp_get_state(a, V, c, pos, None)
+    b = rlx.rlxpp_create(n, 999, 2048)
+    rlx.rlxpp_set_state_ranlux(b, V, c, pos)
+    d2 = torch.empty((n, rest), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(b, d2, rest, rlx.RLXPP_STREAM_MAJOR)
+    ref = oracle.streams(inputs.seeds(n, 31), 2048, first + rest, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(d2.cpu().numpy(), ref["doubles"][:, first:], "continued from the stored form")
+    check_state(rlx, torch, b, ref, "continued from the stored form")
+    rlx.rlxpp_destroy(a)
+    rlx.rlxpp_destroy(b)
+
+
 def test_host_destination_variants(rlx, torch, oracle, nthreads):
     n, per = 2100, 48
     ref = oracle.streams(inputs.seeds(n), 2048, per, want=("doubles", "sums"), nthreads=nthreads)
