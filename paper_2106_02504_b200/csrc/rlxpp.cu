@@ -255,7 +255,7 @@ struct GenArgs {
   // UMMA engine, persistent scheduler: sched[0] = ticket counter, sched[1 + tile] = finished chunks
   u32* sched;
   u32 n_tiles, n_chunks;
-  u64 chunk_len;      // draws per chunk (a multiple of 12 when n_chunks > 1)
+  u64 chunk_len;      // draws per chunk (a multiple of 96 = 8 blocks when n_chunks > 1)
   u32 kexp = kExp16;  // see arith.cuh: a launch parameter on purpose
   // UMMA engine, aligned stream-major stores: tensor map of out (StreamMajorStage)
   alignas(64) CUtensorMap tmap;
@@ -584,7 +584,7 @@ __device__ __forceinline__ void to_ranlux_hot(const u32 (&x)[18], u32 (&v)[18], 
 // handed out in order and sched[1 + tile] counts the chunks of it that are finished (state written
 // back).  With n_chunks == 1 this is a plain grid-stride loop over tiles; with more, the grid's last
 // partial wave shrinks from a whole tile's work to one chunk's (cfg4 / cfg5: 2,048 tiles over
-// 148 x 5 CTAs).  A CTA that waits for chunk c - 1 of its tile waits for an EARLIER ticket, which a
+// 148 x 4 CTAs).  A CTA that waits for chunk c - 1 of its tile waits for an EARLIER ticket, which a
 // resident CTA holds: no deadlock whatever the number of resident CTAs.
 template <int MODE, bool ALIGNED, int OUT = kF64>
 __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(const __grid_constant__ GenArgs a) {

@@ -589,6 +589,76 @@ def test_stream_major_rows_of_any_length(rlx, torch, oracle, nthreads, blocks):
     rlx.rlxpp_destroy(h)
 
 
+@pytest.mark.parametrize("case", [0, 1, 2, 3, 4, 5])
+def test_random_call_sequences_against_the_oracle(rlx, torch, oracle, nthreads, case):
+    """Differential test of the whole C ABI on one handle: a seeded random sequence of skips (uniform and per
+    stream), and generate calls of every output form, layout and count (multiples of 12, of 96, odd counts, 1),
+    each compared with the oracle at the streams' absolute draw positions; the state at the end.  Catches
+    anything that depends on what the previous call left behind (cursor bookkeeping, the aligned fast paths,
+    chunk plans, staging buffers)."""
+    rng = np.random.default_rng(1000 + case)
+    n = int(rng.choice([1, 31, 128, 3 * 128 + 77, 1000]))
+    p = int(rng.choice([2048, 2048, 389, 24]))
+    seed0 = int(rng.integers(1, 1 << 40))
+    seeds = inputs.seeds(n, seed0)
+    g = np.zeros(n, dtype=np.uint64)  # draws consumed so far, per stream
+    h = rlx.rlxpp_create(n, seed0, p)
+    for step in range(14):
+        op = rng.choice(["doubles", "u48", "floats", "normal", "reduce", "skip", "skip_each"])
+        what = f"case {case} step {step} {op} (n = {n}, p = {p})"
+        if op == "skip":
+            d = int(rng.choice([0, 1, 11, 12, 13, 1000, (1 << 40) + 5]))
+            rlx.rlxpp_skip(h, d)
+            g += np.uint64(d)
+            continue
+        if op == "skip_each":
+            d = inputs.splitmix64(int(rng.integers(1 << 30)), n) % np.uint64(rng.choice([2, 12, 5000]))
+            rlx.rlxpp_skip_each(h, torch.from_numpy(d.view(np.int64)).cuda())
+            g += d
+            continue
+        per = int(rng.choice([1, 5, 12, 24, 96, 97, 108, 12 * 23, 12 * 16, 250]))
+        sm = bool(rng.integers(0, 2))
+        lay = rlx.RLXPP_STREAM_MAJOR if sm else rlx.RLXPP_INTERLEAVED
+        shape = (lambda k: (n, k) if sm else (k, n))
+        rows = (lambda t: t.cpu().numpy() if sm else t.cpu().numpy().T)
+        if op == "reduce":
+            S = torch.empty(n, dtype=torch.float64, device="cuda")
+            Q = torch.empty(n, dtype=torch.float64, device="cuda")
+            rlx.rlxpp_generate_reduce(h, S, Q, per)
+            ref = oracle.streams(seeds, p, per, skips=g, want=("sums",), nthreads=nthreads)
+            assert_bits_equal(S.cpu().numpy(), ref["sum"], what + " sum")
+            assert_bits_equal(Q.cpu().numpy(), ref["sumsq"], what + " sumsq")
+        elif op == "normal":
+            out = torch.empty(shape(per), dtype=torch.float64, device="cuda")
+            rlx.rlxpp_generate_normal(h, out, per, lay)
+            odd = (g & np.uint64(1)).astype(np.int64)
+            k = oracle.streams(seeds, p, per + 2 + (per & 1), skips=g - odd.astype(np.uint64), want=("ints",), nthreads=nthreads)["ints"]
+            z = oracle.normals(k)
+            want = np.stack([z[i, odd[i]:odd[i] + per] for i in range(n)])
+            assert_within_ulps(rows(out), want, NORMAL_ULPS, what)
+        else:
+            ref = oracle.streams(seeds, p, per, skips=g, want=("ints", "doubles"), nthreads=nthreads)
+            if op == "doubles":
+                out = torch.empty(shape(per), dtype=torch.float64, device="cuda")
+                rlx.rlxpp_generate_doubles(h, out, per, lay)
+                assert_bits_equal(rows(out), ref["doubles"], what)
+            elif op == "u48":
+                out = torch.empty(shape(per), dtype=torch.int64, device="cuda")
+                rlx.rlxpp_generate_u48(h, out, per, lay)
+                assert np.array_equal(rows(out).view(np.uint64), ref["ints"]), what
+            else:
+                out = torch.empty(shape(2 * per), dtype=torch.float32, device="cuda")
+                rlx.rlxpp_generate_floats(h, out, 2 * per, lay)
+                lo = (ref["ints"] & np.uint64(0xFFFFFF)).astype(np.float32) * np.float32(2.0**-24)
+                hi = (ref["ints"] >> np.uint64(24)).astype(np.float32) * np.float32(2.0**-24)
+                want = np.stack([lo, hi], axis=-1).reshape(n, 2 * per)
+                assert np.array_equal(rows(out).view(np.uint32), want.view(np.uint32)), what
+        g += np.uint64(per)
+    ref = oracle.streams(seeds, p, 0, skips=g, want=("state",), nthreads=nthreads)
+    check_state(rlx, torch, h, ref, f"case {case} final")
+    rlx.rlxpp_destroy(h)
+
+
 def test_generic_multiplier_streams(rlx, torch, oracle, nthreads):
     """A luxury level without baked-in rows (p = 100) runs the full multiply9x9 + mod_m kernels."""
     assert not rlx.rlxpp_has_fixed_multiplier(100)
