@@ -145,6 +145,20 @@ def oracle_sample_rate(n_per, p, target_cpu_seconds=15.0):
     return n * n_per / dt, cores, n, dt
 
 
+def oracle_one_core_rate(n_per, p, target_seconds=2.0):
+    """The same on ONE host thread ('at 1 core and at all cores'), a short sample."""
+    import oracle
+    from paper_2106_02504_b200 import inputs
+    n = 8
+    while True:
+        t0 = time.perf_counter()
+        oracle.streams(inputs.seeds(n), p, n_per, want=("doubles",), nthreads=1)
+        dt = time.perf_counter() - t0
+        if dt >= 0.5 * target_seconds or n >= 1 << 16:
+            return n * n_per / dt, n, dt
+        n = int(min(max(2 * n, n * target_seconds / max(dt, 1e-4)), 1 << 16))
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle (oracle/), unmodified, on the host cores; each step is a
     bounded sample of the workload (same p, same doubles per stream, fewer streams)."""
@@ -490,8 +504,11 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu:
         per = n_per if args.workload != "cfg2" else 12 * 16
         v, cores, ns, dt = oracle_sample_rate(per, p)
+        v1, n1, dt1 = oracle_one_core_rate(per, p)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{ns} of {n_streams} streams x {per} doubles (seeding included), {dt:.2f} s wall on {cores} threads"}
+               "sample": f"{ns} of {n_streams} streams x {per} doubles (seeding included), {dt:.2f} s wall on {cores} threads",
+               "one_core": {"value": v1, "unit": UNIT, "ns_per_double": 1e9 / v1,
+                            "sample": f"{n1} streams x {per} doubles, {dt1:.2f} s on 1 thread"}}
 
     if rank == 0:
         line = {
