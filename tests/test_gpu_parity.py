@@ -158,12 +158,46 @@ def test_cfg3_interleaved_small(rlx, torch, oracle, nthreads):
     check_state(rlx, torch, h, ref, "cfg3 small")
 
 
+_CFG3_CHECKSUMS = {}
+
+
+def cfg3_oracle_checksums(oracle, nthreads, n, per, p=2048):
+    """Per draw index k, over ALL n streams: the wrapping sum of the 48-bit integers and the wrapping sum weighted
+    with 2 i + 1 (i = stream), from the oracle alone (chunks of 2^16 streams; computed once per session)."""
+    key = (n, per, p)
+    if key not in _CFG3_CHECKSUMS:
+        s1 = np.zeros(per, np.uint64)
+        s2 = np.zeros(per, np.uint64)
+        step = 1 << 16
+        with np.errstate(over="ignore"):
+            for lo in range(0, n, step):
+                cnt = min(step, n - lo)
+                k = oracle.streams(inputs.seeds(n)[lo:lo + cnt], p, per, want=("ints",), nthreads=nthreads)["ints"]
+                w = (np.arange(lo, lo + cnt, dtype=np.uint64) * np.uint64(2) + np.uint64(1))[:, None]
+                s1 += k.sum(axis=0, dtype=np.uint64)
+                s2 += (k * w).sum(axis=0, dtype=np.uint64)
+        _CFG3_CHECKSUMS[key] = (s1, s2)
+    return _CFG3_CHECKSUMS[key]
+
+
+def gpu_checksums_interleaved(torch, out, n, per):
+    s1 = torch.zeros(per, dtype=torch.int64, device="cuda")
+    s2 = torch.zeros(per, dtype=torch.int64, device="cuda")
+    w_all = torch.arange(n, dtype=torch.int64, device="cuda") * 2 + 1
+    for lo in range(0, per, 64):
+        k = (out[lo:lo + 64] * 2.0**48).to(torch.int64)  # exact: 48-bit integers
+        s1[lo:lo + 64] = k.sum(dim=1)
+        s2[lo:lo + 64] = (k * w_all[None, :]).sum(dim=1)
+    return s1.cpu().numpy().view(np.uint64), s2.cpu().numpy().view(np.uint64)
+
+
 @pytest.mark.parametrize("layout", ["interleaved", "stream_major"])
 def test_cfg3_full_size_sampled(rlx, torch, oracle, nthreads, layout):
     """BASELINE.json configs[2] in bench.py's launch configuration: 2^20 streams x 1,536 doubles,
     12.9 GB, interleaved (the config's layout) and stream-major (bench.py --layout stream_major).  Sampled
     streams (first and last blocks, a stride through the rest) are compared in full; the whole array is
-    checked for range and lattice on the device."""
+    checked for range and lattice on the device, and through two 64-bit checksums per draw index against the
+    oracle's checksums of all 2^20 streams."""
     n, per = 1 << 20, 1536
     h = rlx.rlxpp_create(n, 1, 2048)
     il = layout == "interleaved"
@@ -182,6 +216,23 @@ def test_cfg3_full_size_sampled(rlx, torch, oracle, nthreads, layout):
         assert bool((blk >= 0).all()) and bool((blk < 1).all())
         sc = blk * 2.0**48
         assert bool((sc == sc.floor()).all())
+    # every one of the 1.6 G doubles: two 64-bit checksums per draw index against the oracle's
+    s1 = torch.zeros(per, dtype=torch.int64, device="cuda")
+    s2 = torch.zeros(per, dtype=torch.int64, device="cuda")
+    w_all = torch.arange(n, dtype=torch.int64, device="cuda") * 2 + 1
+    if il:
+        for lo in range(0, per, 64):
+            k = (out[lo:lo + 64] * 2.0**48).to(torch.int64)  # exact: 48-bit integers
+            s1[lo:lo + 64] = k.sum(dim=1)
+            s2[lo:lo + 64] = (k * w_all[None, :]).sum(dim=1)
+    else:
+        for lo in range(0, n, 1 << 15):
+            k = (out[lo:lo + (1 << 15)] * 2.0**48).to(torch.int64)
+            s1 += k.sum(dim=0)
+            s2 += (k * w_all[lo:lo + (1 << 15), None]).sum(dim=0)
+    o1, o2 = cfg3_oracle_checksums(oracle, nthreads, n, per)
+    assert np.array_equal(s1.cpu().numpy().view(np.uint64), o1), f"cfg3 full, {layout}: sum checksum"
+    assert np.array_equal(s2.cpu().numpy().view(np.uint64), o2), f"cfg3 full, {layout}: weighted checksum"
     V, c, pos, X = gpu_state(rlx, torch, h)
     assert_bits_equal(X[idx], ref["X"], "cfg3 full state")
     assert np.all(pos == 12)
@@ -229,6 +280,9 @@ def test_cfg4_full_size_sampled(rlx, torch, oracle, nthreads, p):
     got = out[:, torch.from_numpy(idx).cuda()].cpu().numpy().T
     ref = oracle.streams(inputs.seeds(n)[idx], p, per, want=("doubles",), nthreads=nthreads)
     assert_bits_equal(got, ref["doubles"], f"cfg4 full p={p}")
+    g1, g2 = gpu_checksums_interleaved(torch, out, n, per)  # all 1.6 G doubles, as in the cfg3 test
+    o1, o2 = cfg3_oracle_checksums(oracle, nthreads, n, per, p)
+    assert np.array_equal(g1, o1) and np.array_equal(g2, o2), f"cfg4 full p={p}: checksums over all streams"
     del out
 
 
