@@ -27,7 +27,7 @@ METRIC = "RANLUX++ p=2048 doubles/sec"
 UNIT = "doubles/s"
 IMAD_PER_ADVANCE = 324  # 18 x 18 products 32x32->64 (81 products 64x64->128)
 IMAD_PER_DOUBLE = 27    # 324 / 12 (one LCG operation per 12 numbers)
-NORMAL_WARP_INST_PER_ADVANCE = 1352  # --output normal: measured, profiles/ncu_r01_umma.md
+NORMAL_WARP_INST_PER_ADVANCE = 835  # --output normal: measured, profiles/ncu_r01_umma.md
 SM_COUNT = 148
 IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles per SMSP, 4 SMSPs
 
@@ -372,8 +372,8 @@ def main():
                     "frac": alu["frac"], "traffic": None, "peak_source": alu["model"] + f" (DESIGN.md); HBM {peak_src}",
                     "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
     if args.output == "normal":
-        # Box-Muller fused into the emission: 1,352 warp instructions per advance (ncu, profiles/ncu_r01_umma.md) make
-        # the kernel issue-bound, not HBM-bound.  Peak = one warp instruction per scheduler and clock.
+        # Box-Muller fused into the emission: 835 warp instructions per advance (ncu, profiles/ncu_r01_umma.md), 342 of
+        # them fp64: the kernel is bound by instruction issue and the fp64 pipe, not by HBM.  Peak = one warp instruction per scheduler and clock.
         winst = units / 12.0 / 32.0 * NORMAL_WARP_INST_PER_ADVANCE / (kernel_ms * 1e-3) / 1e9
         wpeak = SM_COUNT * 4 * sm_max_mhz * 1e6 / 1e9
         roofline = {"bound": "alu", "kernel": kernel.replace("aligned>", "aligned, normal>"), "achieved": winst, "peak": wpeak,

@@ -156,8 +156,9 @@ int rlxpp_generate_floats(rlxpp_t* h, float* out_dev, uint64_t n_per_stream, int
  *   stream's first draw: u0 = k[2i] 2^-48, u1 = k[2i+1] 2^-48, r = sqrt(-2 ln(1 - u0)); the deviate at draw
  *   position 2i is r cos(2 pi u1), at 2i + 1 r sin(2 pi u1).  One deviate per draw position: the call consumes
  *   n_per_stream draws of every stream, any cursor, any count, and interleaves freely with the other generate
- *   calls and with skips (a call that starts or ends inside a pair evaluates that pair twice).  fp64
- *   log / sqrt / sincospi: within 6 ulp of the exact value (the only output form that is not bit-exact);
+ *   calls and with skips (a call that starts or ends inside a pair evaluates that pair twice).  The logarithm
+ *   and the sine / cosine of a turn are the library's own fp64 polynomials (csrc/normal_coeffs.cuh), the square
+ *   root is IEEE: within 6 ulp of the exact value (the only output form that is not bit-exact);
  *   |z| <= sqrt(96 ln 2) = 8.157.  Layouts, ownership and errors as rlxpp_generate_doubles; UMMA engine. */
 int rlxpp_generate_normal(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout);
 

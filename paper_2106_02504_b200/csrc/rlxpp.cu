@@ -22,6 +22,7 @@
 
 #include "../../include/rlxpp.h"
 #include "arith.cuh"
+#include "normal_coeffs.cuh"
 #include "host_bigint.h"
 #include "rows_generated.cuh"
 
@@ -286,20 +287,110 @@ __device__ __forceinline__ double draw_value(const u32 (&v)[18], u32 kexp) {
   return __hiloint2double(__float_as_int(f1), __float_as_int(f0));
 }
 
+// The transcendental part of reading N-1, written for the arguments that occur (CUDA's log / sincospi cost 175
+// instructions per pair with their range checks and general reductions; these cost about half).  Polynomial
+// coefficients: normal_coeffs.cuh (csrc/gen_normal_coeffs.py).  Error against the exact values: ln <= 1 ulp,
+// sin / cos <= 1 ulp, so a deviate is within ~3 ulp (tests: 6 ulp against the long-double oracle).
+namespace nrm {
+// ln(x) for x = 1 - k 2^-48 in [2^-48, 1]: x = 2^e m with m in [sqrt(1/2), sqrt(2)), f = m - 1 (exact),
+// s = f / (2 + f), ln m = 2 s + s z P(z) = f - s (f - z P(z)) with z = s^2: f is exact and dominates, so the rounding
+// of s only enters at second order.  e ln2 is added as hi (32 bits, e hi exact) + lo.  N arguments at once, step by
+// step, so that every constant is set up once per N uses (normal_coeffs.cuh).
+template <int N>
+__device__ __forceinline__ void log_unit(const double (&x)[N], double (&r)[N]) {
+  double f[N], s[N], z[N], p[N], ed[N];
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    int hx = __double2hiint(x[i]) + (0x3ff00000 - 0x3fe6a09e);  // 0x3fe6a09e: high word of sqrt(1/2)
+    ed[i] = (double)((hx >> 20) - 0x3ff);
+    hx = (hx & 0x000fffff) + 0x3fe6a09e;
+    f[i] = __hiloint2double(hx, __double2loint(x[i])) - 1.0;
+  }
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    const double d = 2.0 + f[i];
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));  // ~20 bits; two Newton steps, then one correction of s
+    double t = fma(-d, y, 1.0);
+    y = fma(y, t, y);
+    t = fma(-d, y, 1.0);
+    y = fma(y, t, y);
+    double q = f[i] * y;
+    q = fma(fma(-d, q, f[i]), y, q);
+    s[i] = q;
+    z[i] = q * q;
+  }
+  poly_atanh<N>(z, p);
+#pragma unroll
+  for (int i = 0; i < N; i++) r[i] = fma(ed[i], kLn2Hi, f[i]) - fma(-ed[i], kLn2Lo, s[i] * fma(-z[i], p[i], f[i]));
+}
+// sin and cos of u turns, u = k 2^-48 in [0, 1): x = 2 u (angle pi x), n = round(2 x) in 0 .. 4, r = x - n / 2 exact in
+// [-1/4, 1/4]; the quarter turns are exact sign changes and swaps, so the exact zeros of sin and cos stay exact.
+template <int N>
+__device__ __forceinline__ void sincos_turn(const double (&u)[N], double (&sn)[N], double (&cs)[N]) {
+  double r[N], z[N], ps[N], pc[N];
+  u32 n[N];
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    const double x = u[i] + u[i];
+    const double j = fma(x, 2.0, 0x1.8p52);  // the integer nearest to 2 x sits in the low mantissa bits
+    n[i] = (u32)__double2loint(j);
+    r[i] = fma(j - 0x1.8p52, -0.5, x);
+    z[i] = r[i] * r[i];
+  }
+  poly_sinpi<N>(z, ps);
+  poly_cospi<N>(z, pc);
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    const double s = fma(z[i] * r[i], ps[i], r[i] * kPi);
+    const double c = fma(z[i], pc[i], 1.0);
+    const bool odd = n[i] & 1u;
+    const double so = odd ? c : s, co = odd ? s : c;  // sin(n pi/2 + t), cos(n pi/2 + t) up to sign
+    sn[i] = __hiloint2double(__double2hiint(so) ^ (int)((n[i] & 2u) << 30), __double2loint(so));
+    cs[i] = __hiloint2double(__double2hiint(co) ^ (int)(((n[i] + 1u) & 2u) << 30), __double2loint(co));
+  }
+}
+}  // namespace nrm
+
 // draws J (even) and J + 1 of the block in output form OUT
 template <int OUT, int J>
 __device__ __forceinline__ void draw_pair(const u32 (&v)[18], u32 kexp, double& a, double& b) {
   static_assert(J % 2 == 0, "pairs start at even draws");
   if constexpr (OUT == kNormal) {
-    const double u0 = draw_double<J>(v, kexp), u1 = draw_double<J + 1>(v, kexp);
-    const double r = sqrt(-2.0 * log(1.0 - u0));  // 1 - u0 is exact and in (0, 1]
-    double sn, cs;
-    sincospi(2.0 * u1, &sn, &cs);                 // exact argument: no 2 pi rounding, exact zeros
-    a = r * cs;
-    b = r * sn;
+    const double x[1] = {1.0 - draw_double<J>(v, kexp)}, u1[1] = {draw_double<J + 1>(v, kexp)};  // 1 - u0: exact, in (0, 1]
+    double l[1], sn[1], cs[1];
+    nrm::log_unit<1>(x, l);
+    nrm::sincos_turn<1>(u1, sn, cs);
+    const double r = sqrt(-2.0 * l[0]);
+    a = r * cs[0];
+    b = r * sn[0];
   } else {
     a = draw_value<OUT, J>(v, kexp);
     b = draw_value<OUT, J + 1>(v, kexp);
+  }
+}
+
+// kNormal: the 12 deviates of a block, its six pairs evaluated side by side
+template <int... I>
+__device__ __forceinline__ void draws_of_block(const u32 (&v)[18], u32 kexp, double (&d)[12]) {
+  ((d[I] = draw_double<I>(v, kexp)), ...);
+}
+__device__ __forceinline__ void normal_block(const u32 (&v)[18], u32 kexp, double (&zn)[12]) {
+  double d[12];
+  draws_of_block<0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11>(v, kexp, d);
+  double x[6], u1[6], l[6], sn[6], cs[6];
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    x[i] = 1.0 - d[2 * i];  // exact, in (0, 1]
+    u1[i] = d[2 * i + 1];
+  }
+  nrm::log_unit<6>(x, l);
+  nrm::sincos_turn<6>(u1, sn, cs);
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    const double r = sqrt(-2.0 * l[i]);
+    zn[2 * i] = r * cs[i];
+    zn[2 * i + 1] = r * sn[i];
   }
 }
 
@@ -325,6 +416,16 @@ struct EmitBlock {
   // all 12 draws of block v go to output indices t0 .. t0 + 11 (VEC: t0 is even and p is 16-byte aligned)
   template <bool VEC = true>
   static __device__ __forceinline__ void all(Sink<MODE, OUT>& s, const u32 (&v)[18], u64 t0) {
+    if constexpr (OUT == kNormal && J == 0) {
+      double z[12];
+      normal_block(v, s.kexp, z);
+#pragma unroll
+      for (int j = 0; j < 12; j += 2) {
+        if (MODE == kStoreStreamMajor && VEC) __stcs(reinterpret_cast<double2*>(s.p + t0 + j), make_double2(z[j], z[j + 1]));
+        else { s.emit(t0 + j, z[j]); s.emit(t0 + j + 1, z[j + 1]); }
+      }
+      return;
+    }
     if constexpr (MODE == kStoreStreamMajor && VEC) {
       if constexpr (J % 2 == 0) {  // two draws per 128-bit store (p + t0 is 16-byte aligned: n_per % 12 == 0)
         double2 d2;
@@ -522,12 +623,7 @@ struct StreamMajorStage {
       // the transform is too long to sit in all eight phases (instruction cache): evaluate the block first, then
       // place it; straddling deviates are carried as doubles (cz[j - 4] = z[j])
       double z[12];
-      draw_pair<OUT, 0>(v, kexp, z[0], z[1]);
-      draw_pair<OUT, 2>(v, kexp, z[2], z[3]);
-      draw_pair<OUT, 4>(v, kexp, z[4], z[5]);
-      draw_pair<OUT, 6>(v, kexp, z[6], z[7]);
-      draw_pair<OUT, 8>(v, kexp, z[8], z[9]);
-      draw_pair<OUT, 10>(v, kexp, z[10], z[11]);
+      normal_block(v, kexp, z);
       switch (q) {
         case 0: wait_box(); putd<0, 12, 0>(z); break;
         case 1: putd<0, 12, 96>(z); break;

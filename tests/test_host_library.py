@@ -135,3 +135,36 @@ def test_public_device_header_is_self_contained(tmp_path):
     res = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-I", os.path.join(ROOT, "include"),
                           "-c", src, "-o", str(tmp_path / "example.o")], capture_output=True, text=True)
     assert res.returncode == 0, res.stdout + res.stderr
+
+
+def test_normal_coefficients_header_is_what_its_generator_writes():
+    """csrc/normal_coeffs.cuh (polynomials of rlxpp_generate_normal) is committed; it must be the output of
+    csrc/gen_normal_coeffs.py (mpmath near-minimax fits), and the fits must be as good as the header says."""
+    mp = pytest.importorskip("mpmath")
+    import importlib.util
+    here = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2106_02504_b200", "csrc")
+    spec = importlib.util.spec_from_file_location("gen_normal_coeffs", os.path.join(here, "gen_normal_coeffs.py"))
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
+    text = gen.render()
+    assert text == open(os.path.join(here, "normal_coeffs.cuh")).read()
+    # independent of chebyfit's own error estimate: sin(pi r), cos(pi r) and ln(m) rebuilt in exact arithmetic from the
+    # printed fp64 coefficients (their rounding included): within 2^-54 = a quarter ulp
+    import re
+    polys = {}
+    for name, body in re.findall(r"void poly_(\w+)\(.*?\{(.*?)\n\}", text, re.S):
+        polys[name] = [mp.mpf(float.fromhex(c)) for c in re.findall(r"(-?0x[0-9a-f.]+p[+-]\d+)\)?;", body)]
+    assert {k: len(v) for k, v in polys.items()} == {"sinpi": 7, "cospi": 7, "atanh": 8}
+    horner = lambda cs, z: mp.polyval(cs, z)
+    for t in range(0, 101):
+        r = mp.mpf(t) / 400  # |r| <= 1/4
+        z = r * r
+        s = r * (mp.pi + z * horner(polys["sinpi"], z))
+        c = 1 + z * horner(polys["cospi"], z)
+        assert abs(s - mp.sin(mp.pi * r)) <= mp.mpf(2) ** -54 * max(mp.sin(mp.pi * r), mp.mpf(10) ** -30)
+        assert abs(c - mp.cos(mp.pi * r)) <= mp.mpf(2) ** -54
+        m = mp.sqrt(mp.mpf(1) / 2) + (mp.sqrt(2) - mp.sqrt(mp.mpf(1) / 2)) * t / 100
+        sv = (m - 1) / (m + 1)
+        zz = sv * sv
+        ln = 2 * sv + sv * zz * horner(polys["atanh"], zz)
+        assert abs(ln - mp.log(m)) <= mp.mpf(2) ** -54 * max(abs(mp.log(m)), mp.mpf(10) ** -30)
