@@ -665,6 +665,61 @@ struct StreamMajorStage::Put<OUT, J1, J1, O> {
   static __device__ __forceinline__ void all(StreamMajorStage&, const u32 (&)[18]) {}
 };
 
+// Stream-major stores when the cursors are not all at a block boundary (per-stream skips, draw counts that are
+// not multiples of 12): the rows are shifted against each other by up to 11 doubles, so no TMA box fits, and a thread
+// storing its own 8-byte pieces makes every warp instruction touch 32 rows (measured 100 G doubles/s at the cfg3
+// shape).  Instead the warp parks the block as [32 streams][12 + 1 doubles] in shared memory and copies it out
+// element by element in row order: 32 consecutive lanes write 32 consecutive doubles of 2.67 rows, each lane with the
+// cursor of its element's stream (one shuffle) for the output index and the range mask.
+constexpr u32 kRowStagePitch = 13;                                // doubles; odd: conflict-free 8-byte accesses
+constexpr u32 kRowStageWarpBytes = 32u * kRowStagePitch * 8u;     // 3,328
+struct UnalignedRowStage {
+  u32 buf;        // shared address of this warp's buffer
+  double* row0;   // &out[first stream of the warp][first draw of the item]
+  u64 pitch;      // doubles between rows
+  u32 rows;       // streams of the warp that exist (0 .. 32)
+  u32 kexp;
+  __device__ __forceinline__ void init(uint8_t* stage, double* out_item, u64 warp_first, u64 count, u64 n_per, u32 kexp_) {
+    buf = umma::smem_u32(stage) + (threadIdx.x >> 5) * kRowStageWarpBytes;
+    row0 = out_item + warp_first * n_per;
+    pitch = n_per;
+    rows = warp_first >= count ? 0u : (count - warp_first < 32 ? (u32)(count - warp_first) : 32u);
+    kexp = kexp_;
+  }
+  template <int OUT, int J>
+  __device__ __forceinline__ void park(u32 dst, const u32 (&v)[18]) {
+    if constexpr (J < 12) {
+      double a, b;
+      draw_pair<OUT, J>(v, kexp, a, b);
+      asm volatile("st.shared.f64 [%0], %1;" ::"r"(dst + J * 8), "d"(a) : "memory");
+      asm volatile("st.shared.f64 [%0], %1;" ::"r"(dst + J * 8 + 8), "d"(b) : "memory");
+      park<OUT, J + 2>(dst, v);
+    }
+  }
+  // whole-warp call: block v holds the draws at positions q0 .. q0 + 11 counted from the start of each stream's
+  // current block; position q of a stream with cursor pos is output index q - pos of the item if that is in [0, n)
+  template <int OUT>
+  __device__ __forceinline__ void emit(const u32 (&v)[18], u64 q0, u32 pos, u64 n) {
+    const u32 lane = threadIdx.x & 31u;
+    __syncwarp();  // the copy loop of the previous block has read the buffer
+    park<OUT, 0>(buf + lane * (kRowStagePitch * 8u), v);
+    __syncwarp();
+#pragma unroll
+    for (u32 k = 0; k < 12; k++) {
+      const u32 e = 32u * k + lane;         // element of the [32][12] block in row order
+      const u32 r = (e * 2731u) >> 15;      // e / 12 for e < 384
+      const u32 c = e - 12u * r;
+      const u32 pr = __shfl_sync(0xFFFFFFFFu, pos, r);
+      const u64 t = q0 + c - pr;            // wraps when the draw lies before the stream's cursor: then t >= n
+      if (r < rows && t < n) {
+        double d;
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(d) : "r"(buf + (e + r) * 8u) : "memory");
+        __stcs(row0 + (u64)r * pitch + t, d);
+      }
+    }
+  }
+};
+
 // ----------------------------------------------------------------------------- UMMA engine
 // Same contract as generate_kernel / advance_states_kernel, with multiply9x9 + mod_m done by
 // the tensor core (umma_path.cuh).  One CTA = 128 streams; every thread of the CTA runs the same
@@ -687,6 +742,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
   __shared__ tc::Smem smem;
   constexpr bool kStaged = MODE == kStoreStreamMajor && ALIGNED;
   extern __shared__ __align__(128) uint8_t stage[];  // kStageCtaBytes when kStaged, else none
+  constexpr bool kRowStaged = MODE == kStoreStreamMajor && !ALIGNED;
+  __shared__ __align__(16) uint8_t row_stage[kRowStaged ? 4 * kRowStageWarpBytes : 16];
   tc::Tile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
   tile.setup(smem, a.bmat);
   // the parameter form saves 12 instructions per advance and helps the ALU-bound fused kernel (+5 %); the
@@ -751,10 +808,17 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
     } else if (n > 0) {
       const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
       const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
+      UnalignedRowStage rs;
+      if (kRowStaged) {
+#pragma unroll
+        for (int j = 0; j < 18; j++) v[j] = 0;  // lanes without a current block still take part in the warp's copy
+        rs.init(row_stage, a.out + t0, (u64)tidx * tc::kTile + (threadIdx.x & ~31u), a.count, a.n_per, kexp);
+      }
       if (pos < 12) {
         to_ranlux_exact(x, v, c);
-        if (live) EmitBlock<0, MODE, OUT>::masked(sink, v, 0, pos, n);
+        if (!kRowStaged && live) EmitBlock<0, MODE, OUT>::masked(sink, v, 0, pos, n);
       }
+      if (kRowStaged) rs.emit<OUT>(v, 0, pos, n);  // cursor 12: every position lies before the cursor, nothing is stored
       tile.issue(x);
       // blocks 1 .. smax - 2 lie wholly inside [0, n) for every cursor (last >= smax - 1): no masks
       u64 s = 1;
@@ -765,7 +829,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         tc::reduce_z(z, x);
         tile.issue(x);
         to_ranlux_hot(x, v, c);
-        if (live) EmitBlock<0, MODE, OUT>::template all<false>(sink, v, s * 12 - pos);
+        if (kRowStaged) rs.emit<OUT>(v, s * 12, pos, n);
+        else if (live) EmitBlock<0, MODE, OUT>::template all<false>(sink, v, s * 12 - pos);
       }
 #pragma unroll 1
       for (; s <= smax; s++) {
@@ -780,8 +845,9 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         if (s < smax) tile.issue(x);
         if (take) {
           to_ranlux_hot(x, v, c);
-          if (live) EmitBlock<0, MODE, OUT>::masked(sink, v, s * 12, pos, n);
+          if (!kRowStaged && live) EmitBlock<0, MODE, OUT>::masked(sink, v, s * 12, pos, n);
         }
+        if (kRowStaged) rs.emit<OUT>(v, s * 12, pos, n);  // a stream that ended a block early has all of it past n
       }
       pos = (u32)((u64)pos + n - 12 * last);
     }
