@@ -13,6 +13,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <functional>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -249,6 +250,7 @@ struct GenArgs {
   double* out;   // output of this launch (already offset to its first stream)
   u64 ld;        // INTERLEAVED: doubles between consecutive draws of one stream
   u64 n_per;     // draws per stream
+  u64 pitch = 0; // STREAM_MAJOR: doubles between the rows of consecutive streams (0 = n_per: dense rows)
   double* sum;   // REDUCE: per-stream outputs of this launch (already offset)
   double* sumsq;
   Limbs18 A;
@@ -489,7 +491,7 @@ __global__ void __launch_bounds__(kThreads) generate_kernel(const __grid_constan
   sink.S = 0.0;
   sink.Q = 0.0;
   sink.kexp = MODE == kReduce ? a.kexp : kExp16;
-  sink.p = MODE == kStoreStreamMajor ? a.out + il * a.n_per : (MODE == kStoreInterleaved ? a.out + il : nullptr);
+  sink.p = MODE == kStoreStreamMajor ? a.out + il * (a.pitch ? a.pitch : a.n_per) : (MODE == kStoreInterleaved ? a.out + il : nullptr);
   const u64 n = a.n_per;
   if (ALIGNED) {
     const u64 nblk = n / 12;
@@ -783,7 +785,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
       sink.S = __ldcg(a.sum + il);
       sink.Q = __ldcg(a.sumsq + il);
     }
-    if (MODE == kStoreStreamMajor) sink.p = a.out + il * a.n_per + t0;
+    const u64 pitch = a.pitch ? a.pitch : a.n_per;
+    if (MODE == kStoreStreamMajor) sink.p = a.out + il * pitch + t0;
     else if (MODE == kStoreInterleaved && OUT == kF32)  // 4-byte elements: float il of float row 2 t0
       sink.p = reinterpret_cast<double*>(reinterpret_cast<float*>(a.out) + il + 2 * t0 * a.ld);
     else if (MODE == kStoreInterleaved) sink.p = a.out + il + t0 * a.ld;
@@ -812,7 +815,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
       if (kRowStaged) {
 #pragma unroll
         for (int j = 0; j < 18; j++) v[j] = 0;  // lanes without a current block still take part in the warp's copy
-        rs.init(row_stage, a.out + t0, (u64)tidx * tc::kTile + (threadIdx.x & ~31u), a.count, a.n_per, kexp);
+        rs.init(row_stage, a.out + t0, (u64)tidx * tc::kTile + (threadIdx.x & ~31u), a.count, pitch, kexp);
       }
       if (pos < 12) {
         to_ranlux_exact(x, v, c);
@@ -1287,7 +1290,7 @@ static unsigned tc_slots() {
 // Tensor map of a stream-major output (UMMA engine, aligned): out[count][n_per] doubles viewed as
 // [count][n_per / 16][16], box 32 x 2 x 16, 128-byte swizzle (StreamMajorStage).  n_per >= 16.
 // cuTensorMapEncodeTiled comes from the driver through the runtime (no link against libcuda).
-static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count, uint64_t n_per) {
+static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count, uint64_t n_per, uint64_t pitch) {
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -1302,7 +1305,7 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
   if (n_per >= (1ull << 31) || count >= (1ull << 31))
     return fail(RLXPP_EINVAL, "stream-major output: n_per_stream and the stream count must be below 2^31");
   const cuuint64_t dims[3] = {16, n_per / 16, count};
-  const cuuint64_t strides[2] = {16 * sizeof(double), n_per * sizeof(double)};
+  const cuuint64_t strides[2] = {16 * sizeof(double), pitch * sizeof(double)};
   const cuuint32_t box[3] = {16, 2, 32};
   const cuuint32_t estr[3] = {1, 1, 1};
   const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, out, dims, strides, box, estr,
@@ -1315,7 +1318,7 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
 template <int MODE, int OUT = kF64>
 static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   if (MODE == kStoreStreamMajor && aligned && a.n_per >= kStageCycle) {  // shorter rows never reach the TMA path
-    const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per);
+    const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per, a.pitch ? a.pitch : a.n_per);
     if (rc) return rc;
   }
   const uint64_t n_tiles = (a.count + tc::kTile - 1) / tc::kTile;
@@ -1564,6 +1567,48 @@ static void after_generate(rlxpp_t* h, uint64_t n) {
   h->aligned = h->pos_uniform && h->uniform_pos == 12;
 }
 
+// STREAM_MAJOR, UMMA engine, ONE cursor common to all streams, but the call does not consist of whole blocks (the
+// cursor is inside a block, or the draw count is not a multiple of 12): the rows are still aligned with each
+// other, so the call is cut into  head (up to the block boundary) + whole blocks + tail  and the whole blocks take the
+// aligned path (TMA stores, 780 G doubles/s) with the full rows' pitch; head and tail (< 12 draws each) take the
+// general path.  The aligned path needs 16-byte aligned row pieces: an even pitch and an even head.  Returns -1 if
+// the call does not qualify (the caller then launches it whole).
+static int launch_stream_major_split(const rlxpp_t* h, const GenArgs& a,
+                                     const std::function<int(const GenArgs&, bool)>& launch) {
+  const uint64_t n = a.n_per;
+  if (g_engine.load() != RLXPP_ENGINE_UMMA || !h->pos_uniform || n % 2 || h->uniform_pos % 2) return -1;
+  const uint64_t to_boundary = 12 - h->uniform_pos;  // 0 at a block boundary
+  uint64_t head = to_boundary < n ? to_boundary : n;
+  // rows that are 256-byte multiples: a head of 32 j doubles keeps the aligned path's boxes on the 256-byte granules
+  // the memory system wants (780 instead of 590 G doubles/s for the whole blocks); head = to_boundary + 12 k
+  if (head && n % 32 == 0)
+    for (uint64_t k = 0; k < 8; k++)
+      if ((to_boundary + 12 * k) % 32 == 0 && to_boundary + 12 * k + kStageCycle <= n) {
+        head = to_boundary + 12 * k;
+        break;
+      }
+  const uint64_t mid = (n - head) / 12 * 12, tail = n - head - mid;
+  if (mid < kStageCycle || (head == 0 && tail == 0)) return -1;
+  GenArgs b = a;
+  b.pitch = n;
+  int rc = RLXPP_OK;
+  if (head) {
+    b.n_per = head;
+    rc = launch(b, false);
+  }
+  if (rc == RLXPP_OK) {
+    b.out = a.out + head;
+    b.n_per = mid;
+    rc = launch(b, true);
+  }
+  if (rc == RLXPP_OK && tail) {
+    b.out = a.out + head + mid;
+    b.n_per = tail;
+    rc = launch(b, false);
+  }
+  return rc;
+}
+
 int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout) {
   if (!h) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles: null handle");
   if (layout != RLXPP_STREAM_MAJOR && layout != RLXPP_INTERLEAVED)
@@ -1575,8 +1620,14 @@ int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, i
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = out_dev; a.ld = h->n;
   a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
-  int rc = launch_generate(h->fixed, a, layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved, aligned,
-                           h->stream);
+  int rc = -1;
+  if (layout == RLXPP_STREAM_MAJOR && !aligned)
+    rc = launch_stream_major_split(h, a, [&](const GenArgs& b, bool al) {
+      return launch_generate(h->fixed, b, kStoreStreamMajor, al, h->stream);
+    });
+  if (rc == -1)
+    rc = launch_generate(h->fixed, a, layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved, aligned,
+                         h->stream);
   if (rc) return rc;
   after_generate(h, n_per_stream);
   return RLXPP_OK;
@@ -1609,7 +1660,18 @@ static int generate_other(rlxpp_t* h, void* out_dev, uint64_t n_draws, int layou
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = (double*)out_dev; a.ld = h->n;
   a.n_per = n_draws; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
   const bool aligned = h->aligned && n_draws % 12 == 0;
-  int rc;
+  int rc = -1;
+  if (layout == RLXPP_STREAM_MAJOR && !aligned)
+    rc = launch_stream_major_split(h, a, [&](const GenArgs& b, bool al) {
+      return kind == kU48      ? launch_tc_generate_mode<kStoreStreamMajor, kU48>(b, al, h->stream)
+             : kind == kNormal ? launch_tc_generate_mode<kStoreStreamMajor, kNormal>(b, al, h->stream)
+                               : launch_tc_generate_mode<kStoreStreamMajor, kF32>(b, al, h->stream);
+    });
+  if (rc != -1) {
+    if (rc) return rc;
+    after_generate(h, n_draws);
+    return RLXPP_OK;
+  }
   if (kind == kU48)
     rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor, kU48>(a, aligned, h->stream)
                                       : launch_tc_generate_mode<kStoreInterleaved, kU48>(a, aligned, h->stream);

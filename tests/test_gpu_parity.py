@@ -733,6 +733,50 @@ def test_random_call_sequences_against_the_oracle(rlx, torch, oracle, nthreads, 
     rlx.rlxpp_destroy(h)
 
 
+@pytest.mark.parametrize("skip, counts", [(0, [250, 1000, 12 * 9 + 2]), (4, [500, 130]), (5, [500]), (0, [251, 300]),
+                                          (8, [640, 384]), (4, [1536])])
+def test_stream_major_calls_that_are_not_whole_blocks(rlx, torch, oracle, nthreads, skip, counts):
+    """Stream-major with one common cursor that is inside a block, or a draw count that is not a multiple of 12
+    (rlxpp.cu launch_stream_major_split: head + whole blocks through the aligned path with the row pitch of the
+    whole call + tail; odd cursors / odd counts take the general path whole).  All output forms; ragged tile; the
+    guard band behind the buffer stays untouched."""
+    n = 2 * 128 + 77
+    h = rlx.rlxpp_create(n, 8, 2048)
+    if skip:
+        rlx.rlxpp_skip(h, skip)
+    at = skip
+    for per in counts:
+        for form in ("doubles", "u48", "normal"):
+            buf = torch.full((n * per + 512,), -1.0, dtype=torch.float64, device="cuda")
+            if form == "doubles":
+                rlx.rlxpp_generate_doubles(h, buf, per, rlx.RLXPP_STREAM_MAJOR)
+            elif form == "u48":
+                rlx.rlxpp_generate_u48(h, buf.view(torch.int64), per, rlx.RLXPP_STREAM_MAJOR)
+            else:
+                rlx.rlxpp_generate_normal(h, buf, per, rlx.RLXPP_STREAM_MAJOR)
+            torch.cuda.synchronize()
+            raw = buf.cpu().numpy()
+            got = raw[:n * per].reshape(n, per)
+            assert np.all(raw[n * per:] == -1.0), "wrote behind the output buffer"
+            what = f"skip {skip}, draws {at}..{at + per}, {form}"
+            if form == "normal":
+                lo = at - (at & 1)
+                k = oracle.streams(inputs.seeds(n, 8), 2048, per + 2 + (per & 1), skips=np.full(n, lo, np.uint64),
+                                   want=("ints",), nthreads=nthreads)["ints"]
+                assert_within_ulps(got, oracle.normals(k)[:, at - lo:at - lo + per], NORMAL_ULPS, what)
+            else:
+                ref = oracle.streams(inputs.seeds(n, 8), 2048, per, skips=np.full(n, at, np.uint64),
+                                     want=("ints", "doubles"), nthreads=nthreads)
+                if form == "doubles":
+                    assert_bits_equal(got, ref["doubles"], what)
+                else:
+                    assert np.array_equal(got.view(np.uint64), ref["ints"]), what
+            at += per
+    ref = oracle.streams(inputs.seeds(n, 8), 2048, 0, skips=np.full(n, at, np.uint64), want=("state",), nthreads=nthreads)
+    check_state(rlx, torch, h, ref, "after split calls")
+    rlx.rlxpp_destroy(h)
+
+
 def test_generic_multiplier_streams(rlx, torch, oracle, nthreads):
     """A luxury level without baked-in rows (p = 100) runs the full multiply9x9 + mod_m kernels."""
     assert not rlx.rlxpp_has_fixed_multiplier(100)
