@@ -706,7 +706,7 @@ struct UnalignedRowStage {
     __syncwarp();  // the copy loop of the previous block has read the buffer
     park<OUT, 0>(buf + lane * (kRowStagePitch * 8u), v);
     __syncwarp();
-#pragma unroll
+#pragma unroll 4  // fully unrolled: spills, no faster; hoisting the shuffles out of the loop changes nothing either
     for (u32 k = 0; k < 12; k++) {
       const u32 e = 32u * k + lane;         // element of the [32][12] block in row order
       const u32 r = (e * 2731u) >> 15;      // e / 12 for e < 384
