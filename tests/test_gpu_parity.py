@@ -894,3 +894,20 @@ def test_errors_are_reported_not_swallowed(rlx, torch):
     before = rlx.rlxpp_launch_count()
     rlx.rlxpp_generate_doubles(h, torch.empty(120, dtype=torch.float64, device="cuda"), 12, rlx.RLXPP_STREAM_MAJOR)
     assert rlx.rlxpp_launch_count() == before + 1
+
+
+def test_errors_of_the_widened_calls_and_the_store_probe(rlx, torch):
+    h = rlx.rlxpp_create(64, 1, 2048)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_generate_normal(h, None, 12, rlx.RLXPP_STREAM_MAJOR)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_generate_normal(h, torch.empty(64 * 12, dtype=torch.float64, device="cuda"), 12, 9)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_set_state_ranlux(h, None)
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_measure_hbm_write_pieces(33, 4096, 256, 1)  # rows must be a multiple of 32
+    with pytest.raises(rlx.RlxppError):
+        rlx.rlxpp_measure_hbm_write_pieces(64, 4096, 100, 1)  # pieces are multiples of 16 bytes
+    rlx.rlxpp_generate_normal(h, torch.empty(1, dtype=torch.float64, device="cuda"), 0, rlx.RLXPP_STREAM_MAJOR)  # no-op
+    assert rlx.rlxpp_measure_hbm_write_pieces(1 << 14, 4096, 256, 1) > 1e9  # the probe runs and reports bytes/s
+    rlx.rlxpp_destroy(h)
