@@ -1881,6 +1881,17 @@ int rlxpp_generate_ragged_reduce(rlxpp_t* h, const uint32_t* counts_dev, double*
   return launch_ragged(h, counts_dev, nullptr, 0, sum_dev, sumsq_dev, cooperative, true);
 }
 
+// device buffer and event pair of a probe, released on every return path
+struct ProbeScratch {
+  void* buf = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  ~ProbeScratch() {
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf);
+  }
+};
+
 int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream) {
   if (!imad_per_s || iters <= 0) return fail(RLXPP_EINVAL, "rlxpp_measure_imad_peak: bad argument");
   int rc = check_device();
@@ -1889,11 +1900,12 @@ int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream) {
   int dev = 0, sms = 0;
   CUDA_TRY(cudaGetDevice(&dev));
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  u64* out = nullptr;
-  CUDA_TRY(cudaMalloc(&out, 64));
-  cudaEvent_t e0, e1;
-  CUDA_TRY(cudaEventCreate(&e0));
-  CUDA_TRY(cudaEventCreate(&e1));
+  ProbeScratch ps;
+  CUDA_TRY(cudaMalloc(&ps.buf, 64));
+  CUDA_TRY(cudaEventCreate(&ps.e0));
+  CUDA_TRY(cudaEventCreate(&ps.e1));
+  u64* out = static_cast<u64*>(ps.buf);
+  const cudaEvent_t e0 = ps.e0, e1 = ps.e1;
   const unsigned blocks = (unsigned)sms * 8;  // 8 x 128 threads per SM = 8 warps per scheduler
   const u32 loop = 4096;
   double best = 0.0;
@@ -1908,9 +1920,6 @@ int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream) {
     const double rate = (double)blocks * kThreads * loop * kImadPerIter / (ms * 1e-3);
     if (it >= 2 && rate > best) best = rate;
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(out);
   *imad_per_s = best;
   return RLXPP_OK;
 }
@@ -1923,11 +1932,12 @@ int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s,
   int dev = 0, sms = 0;
   CUDA_TRY(cudaGetDevice(&dev));
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  uint4* buf = nullptr;
-  CUDA_TRY(cudaMalloc(&buf, bytes));
-  cudaEvent_t e0, e1;
-  CUDA_TRY(cudaEventCreate(&e0));
-  CUDA_TRY(cudaEventCreate(&e1));
+  ProbeScratch ps;
+  CUDA_TRY(cudaMalloc(&ps.buf, bytes));
+  CUDA_TRY(cudaEventCreate(&ps.e0));
+  CUDA_TRY(cudaEventCreate(&ps.e1));
+  uint4* buf = static_cast<uint4*>(ps.buf);
+  const cudaEvent_t e0 = ps.e0, e1 = ps.e1;
   double best = 0.0;
   for (int it = 0; it < iters + 2; it++) {
     CUDA_TRY(cudaEventRecord(e0, s));
@@ -1940,9 +1950,6 @@ int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s,
     const double rate = (double)(bytes / 16 * 16) / (ms * 1e-3);
     if (it >= 2 && rate > best) best = rate;
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(buf);
   *bytes_per_s = best;
   return RLXPP_OK;
 }
@@ -1955,11 +1962,12 @@ int rlxpp_measure_hbm_write_pieces(uint64_t rows, uint64_t pitch_bytes, uint32_t
   int rc = check_device();
   if (rc) return rc;
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  uint4* buf = nullptr;
-  CUDA_TRY(cudaMalloc(&buf, rows * pitch_bytes));
-  cudaEvent_t e0, e1;
-  CUDA_TRY(cudaEventCreate(&e0));
-  CUDA_TRY(cudaEventCreate(&e1));
+  ProbeScratch ps;
+  CUDA_TRY(cudaMalloc(&ps.buf, rows * pitch_bytes));
+  CUDA_TRY(cudaEventCreate(&ps.e0));
+  CUDA_TRY(cudaEventCreate(&ps.e1));
+  uint4* buf = static_cast<uint4*>(ps.buf);
+  const cudaEvent_t e0 = ps.e0, e1 = ps.e1;
   const uint64_t written = rows * (pitch_bytes / piece_bytes) * piece_bytes;
   double best = 0.0;
   for (int it = 0; it < iters + 2; it++) {
@@ -1973,9 +1981,6 @@ int rlxpp_measure_hbm_write_pieces(uint64_t rows, uint64_t pitch_bytes, uint32_t
     const double rate = (double)written / (ms * 1e-3);
     if (it >= 2 && rate > best) best = rate;
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(buf);
   *bytes_per_s = best;
   return RLXPP_OK;
 }
