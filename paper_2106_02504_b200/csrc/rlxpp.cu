@@ -251,6 +251,7 @@ struct GenArgs {
   u64 ld;        // INTERLEAVED: doubles between consecutive draws of one stream
   u64 n_per;     // draws per stream
   u64 pitch = 0; // STREAM_MAJOR: doubles between the rows of consecutive streams (0 = n_per: dense rows)
+  u32 f32_boxes = 0;  // INTERLEAVED floats, aligned: tmap describes the float rows (F32RowStage)
   double* sum;   // REDUCE: per-stream outputs of this launch (already offset)
   double* sumsq;
   Limbs18 A;
@@ -722,6 +723,72 @@ struct UnalignedRowStage {
   }
 };
 
+// Interleaved 24-bit floats (rlxpp_generate_floats, aligned cursors).  A float row holds 4 bytes per stream: direct
+// stores are 24 instructions of 128 bytes per warp and advance (measured 700 G draws/s).  Instead the CTA parks a
+// block as [24 float rows][128 streams] in shared memory and ONE thread of the MMA-issuing warp hands it to the TMA
+// as a box of 24 rows x 512 bytes.  No new barrier: the box of block b - 1 is sent from Tile::issue() of advance
+// b + 1, where every thread has fenced its stores and arrived at the hand-off barrier anyway.  Ring of three boxes:
+// block b is written after collect() of advance b, i.e. after the MMA-done mbarrier that the issuing thread committed
+// AFTER waiting (cp.async.bulk.wait_group.read) for the copy of block b - 3.
+constexpr u32 kF32BoxBytes = 24u * 128u * 4u;               // 12,288
+constexpr u32 kF32StageBytes = 3u * kF32BoxBytes + 128u;    // dynamic shared memory (+ alignment)
+struct F32RowStage {
+  u32 base;        // shared address of the ring
+  u32 col;         // this thread's byte offset in a row
+  u32 nfilled;     // blocks parked so far (the same in all threads)
+  u32 nsent;       // blocks handed to the TMA (meaningful in the sending thread only)
+  bool sender;     // lane 0 of the MMA-issuing warp
+  int c0, r0;      // tensor coordinates of the tile's first stream and of the item's first float row
+  const void* tmap;
+  __device__ __forceinline__ void init(uint8_t* stage, const void* tensor_map, u64 tile_first, u64 t0, u32 issuer_warp) {
+    base = (umma::smem_u32(stage) + 127u) & ~127u;
+    col = threadIdx.x * 4u;
+    nfilled = 0;
+    nsent = 0;
+    sender = (threadIdx.x >> 5) == issuer_warp && (threadIdx.x & 31u) == 0;
+    c0 = (int)tile_first;
+    r0 = (int)(2 * t0);
+    tmap = tensor_map;
+  }
+  template <int J>
+  __device__ __forceinline__ void park(u32 dst, const u32 (&v)[18]) {
+    if constexpr (J < 12) {
+      const double d = draw_value<kF32, J>(v, 0u);
+      asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + (2 * J) * 512u), "r"(__double2loint(d)) : "memory");
+      asm volatile("st.shared.b32 [%0], %1;" ::"r"(dst + (2 * J + 1) * 512u), "r"(__double2hiint(d)) : "memory");
+      park<J + 1>(dst, v);
+    }
+  }
+  __device__ __forceinline__ void emit(const u32 (&v)[18]) {
+    park<0>(base + (nfilled % 3u) * kF32BoxBytes + col, v);
+    nfilled++;
+  }
+  // issuing warp, before the MMAs: the boxes sent so far have been read
+  __device__ __forceinline__ void before_mma() {
+    if (sender) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    __syncwarp();
+  }
+  // the CTA's stores to the parked blocks are fenced and handed over: send what is parked and unsent
+  __device__ __forceinline__ void send_parked() {
+    if (sender) {
+      while (nsent < nfilled) {
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap), "r"(c0),
+                     "r"(r0 + 24 * (int)nsent), "r"(base + (nsent % 3u) * kF32BoxBytes)
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        nsent++;
+      }
+    }
+  }
+  // CTA-collective, after the item's last block
+  __device__ __forceinline__ void drain() {
+    umma::fence_proxy_async_smem();
+    __syncthreads();
+    send_parked();
+    if (sender) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+  }
+};
+
 // ----------------------------------------------------------------------------- UMMA engine
 // Same contract as generate_kernel / advance_states_kernel, with multiply9x9 + mod_m done by
 // the tensor core (umma_path.cuh).  One CTA = 128 streams; every thread of the CTA runs the same
@@ -796,18 +863,28 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
       StreamMajorStage sm;
       if (kStaged) sm.init(stage, &a.tmap, (u64)tidx * tc::kTile, kexp, t0);
       const u64 nstaged = nblk & ~(u64)7;  // whole cycles go through the TMA, the rest of a row is stored directly
+      constexpr bool kF32Rows = MODE == kStoreInterleaved && OUT == kF32;
+      const bool f32_boxes = kF32Rows && a.f32_boxes != 0;
+      F32RowStage fs;
+      if (f32_boxes) fs.init(stage, &a.tmap, (u64)tidx * tc::kTile, t0, tile.issuer);
       if (nblk > 0) tile.issue(x);
 #pragma unroll 1
       for (u64 b = 0; b < nblk; b++) {
         u32 z[20];
         tile.collect(z);
         tc::reduce_z(z, x);
-        if (b + 1 < nblk) tile.issue(x);  // the tensor core works on advance b + 2 while block b + 1 is emitted
+        // the tensor core works on advance b + 2 while block b + 1 is emitted
+        if (b + 1 < nblk) {
+          if (f32_boxes) tile.issue(x, [&] { fs.before_mma(); }, [&] { fs.send_parked(); });
+          else tile.issue(x);
+        }
         to_ranlux_hot(x, v, c);
         if (kStaged && b < nstaged) sm.emit<OUT>(v);
+        else if (f32_boxes) fs.emit(v);
         else if (live) EmitBlock<0, MODE, OUT>::all(sink, v, b * 12);
       }
       if (kStaged) sm.drain();
+      if (f32_boxes) fs.drain();
     } else if (n > 0) {
       const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
       const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
@@ -1315,8 +1392,34 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
   return RLXPP_OK;
 }
 
+// Tensor map of an interleaved float output (F32RowStage): float rows of `ld` floats, `count` of them written by this
+// launch, 2 n_per rows; box = 128 streams x 24 rows.  ld must be a multiple of 4 (16-byte row pitch).
+static int encode_f32_rows_map(CUtensorMap* map, float* out, uint64_t count, uint64_t ld, uint64_t rows) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+  if (q != cudaDriverEntryPointSuccess || !fn) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled is not available");
+  const cuuint64_t dims[2] = {count, rows};
+  const cuuint64_t strides[1] = {ld * sizeof(float)};
+  const cuuint32_t box[2] = {128, 24};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = ((EncodeFn)fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr,
+                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled (float rows) failed (%d)", (int)r);
+  return RLXPP_OK;
+}
+
 template <int MODE, int OUT = kF64>
 static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
+  if (MODE == kStoreInterleaved && OUT == kF32 && aligned && a.ld % 4 == 0 && a.count < (1ull << 31) && a.n_per < (1ull << 30)) {
+    const int rc = encode_f32_rows_map(&a.tmap, reinterpret_cast<float*>(a.out), a.count, a.ld, 2 * a.n_per);
+    if (rc) return rc;
+    a.f32_boxes = 1;
+  }
   if (MODE == kStoreStreamMajor && aligned && a.n_per >= kStageCycle) {  // shorter rows never reach the TMA path
     const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per, a.pitch ? a.pitch : a.n_per);
     if (rc) return rc;
@@ -1347,7 +1450,13 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
         if (dev < 64) done.fetch_or(1ull << dev);
       }
     }
-    tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, kStaged ? kStageCtaBytes : 0, s>>>(a);
+    if (a.f32_boxes) {  // 20 KB static + 36 KB of boxes: 4 CTAs per SM still fit
+      CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)kF32StageBytes));
+      CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                    cudaSharedmemCarveoutMaxShared));
+    }
+    tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, kStaged ? kStageCtaBytes : (a.f32_boxes ? kF32StageBytes : 0), s>>>(a);
   } else {
     tc_generate_kernel<MODE, false, OUT><<<grid, tc::kTile, 0, s>>>(a);
   }

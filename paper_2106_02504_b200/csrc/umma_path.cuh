@@ -108,6 +108,13 @@ struct Tile {
 
   // CTA-collective: start  D = Xbytes * B^T  for the 128 states x (any value < 2^576).
   __device__ __forceinline__ void issue(const u32 (&x)[18]) {
+    issue(x, [] {}, [] {});
+  }
+  // before() / after() run in the ISSUING warp (all of its lanes), after the whole CTA has fenced and handed over what
+  // it stored to shared memory, right before and right after the MMAs are issued and committed: the place for other
+  // async-proxy work on the CTA's shared memory that must be ordered with the MMA-done mbarrier (F32RowStage).
+  template <class Before, class After>
+  __device__ __forceinline__ void issue(const u32 (&x)[18], Before&& before, After&& after) {
 #pragma unroll
     for (int g = 0; g < 4; g++)
       asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a_row + (u32)g * kAChunk), "r"(x[4 * g]),
@@ -120,8 +127,10 @@ struct Tile {
     if (SYNC == kSyncArrive) {
       if ((threadIdx.x >> 5) == issuer) {
         asm volatile("bar.sync 1, 128;" ::: "memory");
+        before();
         if (umma::elect_one()) issue_mma();
         __syncwarp();
+        after();
       } else {
         asm volatile("bar.arrive 1, 128;" ::: "memory");
       }

@@ -911,3 +911,32 @@ def test_errors_of_the_widened_calls_and_the_store_probe(rlx, torch):
     rlx.rlxpp_generate_normal(h, torch.empty(1, dtype=torch.float64, device="cuda"), 0, rlx.RLXPP_STREAM_MAJOR)  # no-op
     assert rlx.rlxpp_measure_hbm_write_pieces(1 << 14, 4096, 256, 1) > 1e9  # the probe runs and reports bytes/s
     rlx.rlxpp_destroy(h)
+
+
+@pytest.mark.parametrize("blocks", [1, 2, 3, 4, 7, 40])
+@pytest.mark.parametrize("n", [3 * 128 + 44, 3 * 128 + 45])
+def test_interleaved_floats_through_row_boxes(rlx, torch, oracle, nthreads, blocks, n):
+    """rlxpp_generate_floats, interleaved, aligned cursors (UMMA engine: the CTA's block leaves as one TMA box of
+    24 float rows x 128 streams, three boxes in flight; rlxpp.cu F32RowStage).  1, 2, 3 blocks (fewer than the ring),
+    more; a ragged last tile the tensor map must clip; n not a multiple of 4 takes the direct stores; forced chunks;
+    the guard band stays untouched; two calls in a row."""
+    per = 12 * blocks
+    h = rlx.rlxpp_create(n, 21, 2048)
+    ref = oracle.streams(inputs.seeds(n, 21), 2048, 3 * per, want=("ints", "state"), nthreads=nthreads)
+    want = _floats_of(ref["ints"])  # [n][2 * 3 per]
+    for call in range(3):
+        if call == 2:
+            rlx.rlxpp_set_chunks(2)
+        try:
+            buf = torch.full((2 * per * n + 256,), -1.0, dtype=torch.float32, device="cuda")
+            rlx.rlxpp_generate_floats(h, buf, 2 * per, rlx.RLXPP_INTERLEAVED)
+            torch.cuda.synchronize()
+        finally:
+            rlx.rlxpp_set_chunks(0)
+        raw = buf.cpu().numpy()
+        got = raw[:2 * per * n].reshape(2 * per, n).T
+        assert np.array_equal(got.view(np.uint32), want[:, call * 2 * per:(call + 1) * 2 * per].view(np.uint32)), \
+            f"interleaved floats, {blocks} blocks, n = {n}, call {call}"
+        assert np.all(raw[2 * per * n:] == -1.0), "wrote behind the output buffer"
+    check_state(rlx, torch, h, ref, "interleaved floats")
+    rlx.rlxpp_destroy(h)
