@@ -27,7 +27,11 @@ METRIC = "RANLUX++ p=2048 doubles/sec"
 UNIT = "doubles/s"
 IMAD_PER_ADVANCE = 324  # 18 x 18 products 32x32->64 (81 products 64x64->128)
 IMAD_PER_DOUBLE = 27    # 324 / 12 (one LCG operation per 12 numbers)
-NORMAL_WARP_INST_PER_ADVANCE = 835  # --output normal: measured, profiles/ncu_r01_umma.md
+# Warp instructions the dominant kernel executes per advance of one warp's 32 streams (ncu smsp__inst_executed.sum /
+# (advances / 32) of the committed --set full captures; profiles/ncu_r02_umma.md).  The issue-slot roofline of the
+# kernels that neither HBM nor the tensor pipe binds: one warp instruction per scheduler and clock.
+WARP_INST_PER_ADVANCE = {"normal": 835, "cfg5": 235, "cfg2": 158}
+TRAFFIC_FILE = "profiles/traffic_r02.json"
 SM_COUNT = 148
 IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles per SMSP, 4 SMSPs
 
@@ -50,6 +54,25 @@ def peaks():
             d = json.load(f)
         return d.get("hbm_gbs", 6650.0), d.get("sm_max_mhz", 1965.0), "measured (MEASURED_PEAKS.json)"
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def job_layout(rank, world, n_streams_per_gpu, seed=1):
+    """Weak scaling: the job has world x n_streams_per_gpu streams, rank g owns the contiguous range g and
+    seeds its first stream with seed + first (mod 2^64).  -> (first stream, streams of this rank, seed argument)."""
+    from paper_2106_02504_b200 import shard
+    first, count = shard.stream_range(rank, world, world * n_streams_per_gpu)
+    return first, count, shard.rank_seed(seed, first)
+
+
+def whole_job_rate(units_per_rank, world, ms):
+    """`value`: the units ALL ranks processed divided by the slowest rank's time."""
+    return units_per_rank * world / (ms * 1e-3)
+
+
+def spread(xs):
+    xs = sorted(xs)
+    return {"min": xs[0], "median": xs[len(xs) // 2] if len(xs) % 2 else 0.5 * (xs[len(xs) // 2 - 1] + xs[len(xs) // 2]),
+            "max": xs[-1], "mean": sum(xs) / len(xs), "n": len(xs)}
 
 
 class ClockSampler:
@@ -222,7 +245,10 @@ def main():
     ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--sustained-s", type=float, default=3.0,
+                    help="after the timed region, repeat the step back to back for at least this many seconds with the clock "
+                         "sampler running and report it as `sustained` (0 = skip)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -252,9 +278,8 @@ def main():
     if args.p:
         p = args.p
     # weak scaling: the job has world x n_streams streams, rank g owns the contiguous range g
-    first_stream, my_streams = shard.stream_range(rank, world, world * n_streams)
+    first_stream, my_streams, first_seed = job_layout(rank, world, n_streams)
     assert my_streams == n_streams
-    first_seed = shard.rank_seed(1, first_stream)
     stream = torch.cuda.current_stream()
 
     # ---------------------------------------------------------------- set up the step
@@ -343,11 +368,13 @@ def main():
     per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
     total_ms = shard.max_over_ranks(total_ms, dist, "cuda")
     ms_per_step = total_ms / args.steps
-    value = units * world / (ms_per_step * 1e-3)
+    value = whole_job_rate(units, world, ms_per_step)
 
     # ---------------------------------------------------------------- roofline of the dominant kernel
     hbm_gbs, sm_max_mhz, peak_src = peaks()
     kernel_ms = sum(per_launch_ms) / len(per_launch_ms)  # one launch per step: event pairs bracket single launches
+    launch_spread = spread(per_launch_ms)
+    launch_spread["first"] = per_launch_ms[0]
     imad_nominal = SM_COUNT * IMAD_LANES_PER_CLK_SM * sm_max_mhz * 1e6  # IMAD/s at max clock
     imad_achieved = units * IMAD_PER_DOUBLE / (kernel_ms * 1e-3)
     hbm_achieved = alg_bytes / (kernel_ms * 1e-3) / 1e9
@@ -374,11 +401,11 @@ def main():
     if args.output == "normal":
         # Box-Muller fused into the emission: 835 warp instructions per advance (ncu, profiles/ncu_r01_umma.md), 342 of
         # them fp64: the kernel is bound by instruction issue and the fp64 pipe, not by HBM.  Peak = one warp instruction per scheduler and clock.
-        winst = units / 12.0 / 32.0 * NORMAL_WARP_INST_PER_ADVANCE / (kernel_ms * 1e-3) / 1e9
+        winst = units / 12.0 / 32.0 * WARP_INST_PER_ADVANCE["normal"] / (kernel_ms * 1e-3) / 1e9
         wpeak = SM_COUNT * 4 * sm_max_mhz * 1e6 / 1e9
         roofline = {"bound": "alu", "kernel": kernel.replace("aligned>", "aligned, normal>"), "achieved": winst, "peak": wpeak,
                     "unit": "G warp instructions/s", "frac": winst / wpeak, "traffic": None,
-                    "peak_source": f"{NORMAL_WARP_INST_PER_ADVANCE} warp instructions per advance of 32 streams (ncu, "
+                    "peak_source": f"{WARP_INST_PER_ADVANCE["normal"]} warp instructions per advance of 32 streams (ncu, "
                                    f"smsp__inst_executed) x advances; peak = {SM_COUNT} SMs x 4 schedulers x {sm_max_mhz:.0f} MHz",
                     "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
     roofline["engine"] = args.engine
@@ -393,12 +420,17 @@ def main():
         roofline["tensor"] = {"achieved": tops, "peak": 2.0 * bf16, "unit": "TOP/s (u8 x u8 -> s32)", "frac": tops / (2.0 * bf16),
                               "what": "tcgen05.mma kind::i8 work incl. the K 72->96 and N 72->80 padding; peak = measured "
                                       "bf16 x 2 (the guide's nominal int8 : bf16 ratio)"}
-        if not stores:
-            # no stores: the products run on the tensor pipe, so the contraction's own peak is the roofline;
-            # the north_star IMAD model (which this engine exceeds) stays in `alu` / `doubles_roofline`
-            roofline.update(bound="tensor", achieved=tops, peak=2.0 * bf16, unit="TOP/s", frac=tops / (2.0 * bf16),
-                            peak_source="u8 x u8 -> s32 tcgen05.mma: measured bf16 dense (MEASURED_PEAKS.json) x 2; "
-                                        "15,360 integer ops per advance (M128 x N80 x K96 tile per 128 streams)")
+        if not stores and args.workload in WARP_INST_PER_ADVANCE:
+            # No stores, products on the tensor pipe (far from its peak: see `tensor`): what binds is warp-instruction
+            # issue -- the carry chains of the normalisation, to_ranlux and the fused sums.  Peak = one warp instruction
+            # per scheduler and clock; achieved = measured instructions per advance (ncu) x advances per second.
+            wpa = WARP_INST_PER_ADVANCE[args.workload]
+            winst = units / 12.0 / 32.0 * wpa / (kernel_ms * 1e-3) / 1e9
+            wpeak = SM_COUNT * 4 * sm_max_mhz * 1e6 / 1e9
+            roofline.update(bound="alu", achieved=winst, peak=wpeak, unit="G warp instructions/s", frac=winst / wpeak,
+                            peak_source=f"{wpa} warp instructions per advance of 32 streams (ncu smsp__inst_executed, "
+                                        f"profiles/ncu_r02_umma.md) x advances/s; peak = {SM_COUNT} SMs x 4 schedulers x "
+                                        f"{sm_max_mhz:.0f} MHz (DESIGN.md 6); the tensor pipe's share is in `tensor`")
     roofline["doubles_roofline"] = {"alu": roof_alu, "hbm": (None if roof_hbm == float("inf") else roof_hbm),
                                     "min": min(roof_alu, roof_hbm), "frac": doubles_rate / min(roof_alu, roof_hbm),
                                     "what": "north_star's roofline: the slower of nominal IMAD peak / 27 and HBM peak / 8 B"}
@@ -412,11 +444,43 @@ def main():
             roofline["hbm_write_microbench_peak"] = rlx.rlxpp_measure_hbm_write_peak(8 << 30, 3) / 1e9
         except rlx.RlxppError as e:  # the probes are context, the headline does not depend on them
             roofline["probe_error"] = str(e)
-    traffic_file = os.path.join(ROOT, "profiles", "traffic_r01.json")
+    traffic_file = os.path.join(ROOT, TRAFFIC_FILE)
     if os.path.exists(traffic_file):
         with open(traffic_file) as f:
             key = f"{args.workload}:{args.engine}" + ("" if args.layout == "interleaved" else ":" + args.layout)
             roofline["traffic"] = json.load(f).get(key)
+    # NOT measured by this run: ncu cannot run inside a timed bench; the figure is the committed capture's
+    roofline["traffic_source"] = (f"{TRAFFIC_FILE}: dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed "
+                                  "ncu --set full capture of this kernel (another run of the same build), not this run")
+    roofline["per_launch_ms"] = launch_spread
+
+    # ---------------------------------------------------------------- sustained: the same step for >= 3 s
+    sustained = None
+    if args.sustained_s > 0 and rank == 0:
+        torch.cuda.synchronize()
+        est = max(launch_spread["median"], 1e-3)
+        block = max(1, int(100.0 / est))          # ~0.1 s of launches between events
+        n_blocks = max(3, int(args.sustained_s * 1e3 / (block * est)) + 1)
+        s_sampler = ClockSampler(local)
+        sev = [torch.cuda.Event(enable_timing=True) for _ in range(n_blocks + 1)]
+        t0 = time.perf_counter()
+        sev[0].record(stream)
+        for b in range(n_blocks):
+            for _ in range(block):
+                step()
+            sev[b + 1].record(stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        s_clocks = s_sampler.stop()
+        blocks_ms = [sev[b].elapsed_time(sev[b + 1]) / block for b in range(n_blocks)]
+        s_ms = sev[0].elapsed_time(sev[-1]) / (n_blocks * block)
+        sustained = {"value": units / (s_ms * 1e-3), "unit": UNIT, "launches": n_blocks * block, "wall_s": wall,
+                     "ms_per_launch": s_ms, "ms_per_launch_by_block": spread(blocks_ms),
+                     "first_block_ms": blocks_ms[0], "last_block_ms": blocks_ms[-1],
+                     "frac_of_burst_value": units / (s_ms * 1e-3) / (units / (kernel_ms * 1e-3)),
+                     "roofline_frac": roofline["frac"] * kernel_ms / s_ms, "clocks": s_clocks,
+                     "what": f"the timed step repeated back to back for >= {args.sustained_s:g} s on this rank, CUDA events every "
+                             f"{block} launches; NVML clocks / power / reasons sampled throughout"}
 
     # ---------------------------------------------------------------- the other engine, same workload (context)
     compare = None
@@ -490,13 +554,18 @@ def main():
         e2e_step()  # warm-up (also pins / allocates the staging buffers' pages)
         barrier()
         t0 = time.perf_counter()
+        e2e_each = []
         for _ in range(args.e2e_steps):
-            e2e_step()
+            t1 = time.perf_counter()
+            e2e_step()  # returns when the host buffer is complete
+            e2e_each.append(time.perf_counter() - t1)
         barrier()
         dt = time.perf_counter() - t0
         dt = shard.max_over_ranks(dt, dist, "cuda")
+        each = spread([units / t for t in e2e_each])
         e2e = {"value": units * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": args.e2e_steps,
+               "per_step_this_rank": {"min": each["min"], "median": each["median"], "max": each["max"], "unit": UNIT},
                "what": "rlxpp_create (seed kernel) + rlxpp_generate_*_host into pinned host memory + rlxpp_destroy, wall clock"}
 
     # ---------------------------------------------------------------- oracle on the host cores
@@ -523,7 +592,9 @@ def main():
                                                                   "compute-bound; working set is registers"),
                        "parallelism": f"streams sharded over {world} GPU(s), no collective"},
             "lcg_advances_per_s": value / 12.0,
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "value_from_median_launch": units * world / (launch_spread["median"] * 1e-3),
+            "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks,
             "other_engine": compare,
         }
         if devapi is not None:

@@ -25,6 +25,14 @@
  *     and the calls return WITHOUT synchronising, except the *_host variants, which
  *     return after the host buffer is complete.
  *   - 576-bit integers cross the boundary as 9 little-endian uint64_t.
+ *   - Threads and processes.  The library is built for ONE PROCESS PER GPU (streams are independent,
+ *     a rank owns a contiguous range of them; no collective).  A handle belongs to the device that was current at
+ *     rlxpp_create and is single-threaded: it owns one scheduler buffer and one pair of staging buffers, so two
+ *     host threads must not call into the same handle at the same time (different handles are fine).
+ *     rlxpp_set_engine, rlxpp_set_chunks and the rare-path counters are process-wide.  Caches keyed by
+ *     (device, p) -- the byte matrices, the power tables -- live for the life of the process.
+ *   - After a failed rlxpp_generate_*_host call the streams are in a defined but partly advanced state (earlier
+ *     stream ranges have drawn, later ones have not); re-import states or destroy the handle.
  */
 #ifndef RLXPP_H
 #define RLXPP_H
@@ -182,12 +190,39 @@ int rlxpp_device_view(rlxpp_t* h, struct rlxpp_view* out_host);
 /* Ragged generation, written with that device API: stream i draws counts_dev[i] doubles (uint32,
  * device pointer, n_streams entries).  out_dev[i * ld + t] = draw t of stream i (ld >= max count;
  * entries beyond a stream's count are left untouched); the _reduce form keeps S = S + d and
- * Q = fma(d, d, Q) per stream in draw order (sumsq_dev may be NULL).  cooperative != 0 uses the
- * warp-cooperative advance (draw_coop), 0 the paper's per-thread advance (draw); results are identical.
+ * Q = fma(d, d, Q) per stream in draw order (sumsq_dev may be NULL).  cooperative = 1 uses the
+ * warp-cooperative advance (draw_coop), 0 the paper's per-thread advance (draw), 2 alternates the two from
+ * draw to draw on the same generator (they mix freely); results are identical.
  * State and cursors are updated; the draws are the ones rlxpp_generate_doubles would give. */
 int rlxpp_generate_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out_dev, uint64_t ld, int cooperative);
 int rlxpp_generate_ragged_reduce(rlxpp_t* h, const uint32_t* counts_dev, double* sum_dev, double* sumsq_dev,
                                  int cooperative);
+
+/* ---- Rare-path counters (debug / test instrumentation of the hot kernels) ------------------------------
+ * mod_m ("smaller than m in all cases") and the conversion back to RANLUX numbers (line 39)
+ * run in the hot kernels as fast forms that take the overwhelmingly likely case and hand everything else to
+ * the exact code.  Each condition that does so is counted per device, per advance of one stream,
+ * in the cold path only:
+ *   [RLXPP_RARE_FOLD_BORROW]   folding the bits above 2^576: the borrow of "- hi" leaves limb 1
+ *   [RLXPP_RARE_FOLD_CARRY]    ... the carry of "+ hi 2^240" leaves limb 9
+ *   [RLXPP_RARE_FOLD_TOP]      ... top limb all ones (the folded value may be >= m)
+ *   [RLXPP_RARE_RANLUX_CARRY]  to_ranlux: carry out of the 8-limb addition X + (X >> 336)
+ *   [RLXPP_RARE_RANLUX_NEAR]   to_ranlux: |u - w| <= 1, u = bits 304..335, w = bits 544..575 of X
+ *   [RLXPP_RARE_RANLUX_UMAX]   to_ranlux: u = 2^32 - 1
+ *   [RLXPP_RARE_RANLUX_V0]     to_ranlux: subtracting the carry would borrow out of limb 0
+ *   [RLXPP_RARE_RANLUX_THIRD]  the exact conversion gave reading D4's third combination (T = Xh, c = 1)
+ * rlxpp_rare_counts synchronises the current device, copies the RLXPP_RARE_KINDS counters to out_host (may be
+ * NULL) and zeroes them if reset != 0.  Process-wide per device; not meant for concurrent use.  Errors: ECUDA. */
+#define RLXPP_RARE_FOLD_BORROW 0
+#define RLXPP_RARE_FOLD_CARRY 1
+#define RLXPP_RARE_FOLD_TOP 2
+#define RLXPP_RARE_RANLUX_CARRY 3
+#define RLXPP_RARE_RANLUX_NEAR 4
+#define RLXPP_RARE_RANLUX_UMAX 5
+#define RLXPP_RARE_RANLUX_V0 6
+#define RLXPP_RARE_RANLUX_THIRD 7
+#define RLXPP_RARE_KINDS 8
+int rlxpp_rare_counts(uint64_t* out_host, int reset);
 
 uint64_t rlxpp_n_streams(const rlxpp_t* h);
 /* 1 if the kernels with immediate multipliers serve this luxury level */

@@ -22,6 +22,8 @@
 //              block in the same pass (state and spare block live in local memory / registers).  Each
 //              lane uses its spare when its own block runs out, so the warp pays one advance pass per
 //              12 draws per lane whatever the cursors are.
+// The two mix freely on one Stream (draw_coop() in converged code, draw() inside a divergent branch): draw()
+// enters a spare block that draw_coop() has made instead of advancing again.
 //
 // The advance here is the paper's own formulation (multiply9x9, then mod_m) on 32-bit
 // limbs with the multiplier a^p as 18 runtime limbs, any luxury level p.  (The library's bulk kernels
@@ -413,7 +415,13 @@ class Stream {
   // Next 48-bit integer of the stream (reading D6), per-thread advance.
   __device__ __forceinline__ uint64_t draw_u48() {
     if (pos_ == 12u) {
-      advance(x_, v_);
+      if (spare_) {  // draw_coop() already made the next block: enter it (draw and draw_coop mix freely)
+#pragma unroll
+        for (int j = 0; j < 18; j++) { x_[j] = xs_[j]; v_[j] = vs_[j]; }
+        spare_ = 0;
+      } else {
+        advance(x_, v_);
+      }
       pos_ = 0;
     }
     return take();

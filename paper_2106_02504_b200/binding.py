@@ -62,6 +62,7 @@ _SIGNATURES = {
                                              ctypes.c_int]),
     "rlxpp_generate_ragged_reduce": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                                     ctypes.c_int]),
+    "rlxpp_rare_counts": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]),
     "rlxpp_n_streams": (ctypes.c_uint64, [ctypes.c_void_p]),
     "rlxpp_has_fixed_multiplier": (ctypes.c_int, [ctypes.c_uint32]),
     "rlxpp_launch_count": (ctypes.c_uint64, []),
@@ -212,12 +213,12 @@ def rlxpp_device_view(h: Handle) -> RlxppView:
     return v
 
 
-def rlxpp_generate_ragged(h: Handle, counts_dev, out_dev, ld: int, cooperative: bool = True):
+def rlxpp_generate_ragged(h: Handle, counts_dev, out_dev, ld: int, cooperative=True):
     _check(load().rlxpp_generate_ragged(h.ptr, _ptr(counts_dev), _ptr(out_dev), ld, int(cooperative)),
            "rlxpp_generate_ragged")
 
 
-def rlxpp_generate_ragged_reduce(h: Handle, counts_dev, sum_dev, sumsq_dev, cooperative: bool = True):
+def rlxpp_generate_ragged_reduce(h: Handle, counts_dev, sum_dev, sumsq_dev, cooperative=True):
     _check(load().rlxpp_generate_ragged_reduce(h.ptr, _ptr(counts_dev), _ptr(sum_dev), _ptr(sumsq_dev), int(cooperative)),
            "rlxpp_generate_ragged_reduce")
 
@@ -273,6 +274,17 @@ def rlxpp_set_chunks(n_chunks: int):
 
 def rlxpp_get_engine() -> int:
     return int(load().rlxpp_get_engine())
+
+
+RLXPP_RARE_KINDS = 8
+RLXPP_RARE_NAMES = ("fold_borrow", "fold_carry", "fold_top", "ranlux_carry", "ranlux_near", "ranlux_umax", "ranlux_v0",
+                    "ranlux_third")
+
+
+def rlxpp_rare_counts(reset: bool = False) -> np.ndarray:
+    out = np.zeros(RLXPP_RARE_KINDS, np.uint64)
+    _check(load().rlxpp_rare_counts(out.ctypes.data, int(reset)), "rlxpp_rare_counts")
+    return out
 
 
 def rlxpp_n_streams(h: Handle) -> int:

@@ -125,7 +125,10 @@ struct Fixed {
     FixedMultiplier<P>::mul(x, E, e9, O, o9);
     merge_eo(E, e9, O, o9, z);
     fold_fast(z, x, rare);
-    if (__builtin_expect(rare != 0, 0)) exact_fold(z, x);
+    if (__builtin_expect(rare != 0, 0)) {
+      count_rare(fold_rare_mask(z[0], z[1], z[7], z[8], z[9], z[17], z[18], z[19]));
+      exact_fold(z, x);
+    }
   }
   // x <- A x mod m and v, c <- to_ranlux(x)
   __device__ __forceinline__ void advance_block(u32 (&x)[18], u32 (&v)[18], u32& c) const {
@@ -135,7 +138,13 @@ struct Fixed {
     merge_eo(E, e9, O, o9, z);
     fold_fast(z, x, rare);
     to_ranlux_fast(x, v, c, rare);
-    if (__builtin_expect(rare != 0, 0)) exact_fold_to_ranlux(z, x, v, &c);
+    if (__builtin_expect(rare != 0, 0)) {
+      // to_ranlux_fast saw the right x only if the fold was exact: its conditions count only then
+      const u32 fm = fold_rare_mask(z[0], z[1], z[7], z[8], z[9], z[17], z[18], z[19]);
+      exact_fold_to_ranlux(z, x, v, &c);
+      const u32 rm = ranlux_rare_mask(x, v, c);
+      count_rare(fm ? fm | (rm & (1u << kRareRanluxThird)) : rm);
+    }
   }
 };
 struct Generic {
@@ -796,7 +805,10 @@ struct F32RowStage {
 __device__ __forceinline__ void to_ranlux_hot(const u32 (&x)[18], u32 (&v)[18], u32& c) {
   u32 rare = 0;
   to_ranlux_fast(x, v, c, rare);
-  if (__builtin_expect(rare != 0, 0)) to_ranlux_exact(x, v, c);  // inline: a call would force x, v into local memory
+  if (__builtin_expect(rare != 0, 0)) {
+    to_ranlux_exact(x, v, c);  // inline: a call would force x, v into local memory
+    count_rare(ranlux_rare_mask(x, v, c));
+  }
 }
 
 // Persistent grid with a ticket scheduler.  A work item = (tile of 128 streams, chunk of
@@ -1108,8 +1120,9 @@ __global__ void __launch_bounds__(kThreads) import_ranlux_kernel(uint4* __restri
 // (one state per thread, threads consume numbers at their own pace).  Written entirely
 // with the public per-thread API of include/rlxpp_device.cuh, of which it is the reference use:
 // COOP = draw_coop() (one advance pass per warp and 12 draws whatever the cursors), else draw()
-// (the paper's per-thread advance, which diverges).
-template <bool COOP, bool REDUCE>
+// (the paper's per-thread advance, which diverges); COOP = 2 alternates the two from draw to draw on the same Stream
+// (they mix freely: a spare block made by draw_coop() is entered by draw()).
+template <int COOP, bool REDUCE>
 __global__ void __launch_bounds__(kThreads) ragged_kernel(const rlxpp_view_t view, const u32* __restrict__ counts,
                                                           double* __restrict__ out, u64 ld, double* __restrict__ sum,
                                                           double* __restrict__ sumsq) {
@@ -1126,7 +1139,7 @@ __global__ void __launch_bounds__(kThreads) ragged_kernel(const rlxpp_view_t vie
     for (u32 t = 0; t < maxc; t++) {
       const unsigned mask = __ballot_sync(0xFFFFFFFFu, t < cnt);
       if (t < cnt) {
-        const double d = g.draw_coop(mask);
+        const double d = (COOP == 2 && (t & 1u)) ? g.draw() : g.draw_coop(mask);
         if (REDUCE) { S = S + d; Q = __fma_rn(d, d, Q); }
         else row[t] = d;
       }
@@ -1224,6 +1237,19 @@ static void build_tables(uint32_t p, Tables& t, bool with_pow_tables) {
     cur.to_u32x18(&t.tabG[b * 18]);
     cur = host::mulmod(cur, cur);
   }
+}
+
+// The tables depend on p only (about 230 host modular products): built once per luxury level and process.
+static const Tables& cached_tables(uint32_t p) {
+  static std::mutex mu;
+  static std::vector<Tables*> cache;  // never freed: handles keep references
+  std::lock_guard<std::mutex> lock(mu);
+  for (const Tables* t : cache)
+    if (t->p == p) return *t;
+  Tables* t = new Tables();
+  build_tables(p, *t, true);
+  cache.push_back(t);
+  return *t;
 }
 
 // Shared-memory image of the byte matrix B of the UMMA engine: B[n][k] = byte n of
@@ -1354,31 +1380,52 @@ static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_
   *n_chunks = (uint32_t)((n_per + len - 1) / len);
 }
 
-static unsigned tc_slots() {
-  static unsigned slots = 0;
-  if (slots == 0) {
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    slots = (unsigned)sms * tc::kCtasPerSm;
-  }
+static unsigned tc_slots() {  // resident CTAs of the persistent UMMA kernels on the CURRENT device
+  static std::atomic<unsigned> cache[64];
+  int dev = 0, sms = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess) dev = 0;
+  if (dev >= 0 && dev < 64 && cache[dev].load()) return cache[dev].load();
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const unsigned slots = (unsigned)sms * tc::kCtasPerSm;
+  if (dev >= 0 && dev < 64) cache[dev].store(slots);
   return slots;
+}
+
+// cuTensorMapEncodeTiled from the driver through the runtime (no link against libcuda); looked up once.
+typedef CUresult (*TensorMapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                      const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                      CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static int tensor_map_encoder(TensorMapEncodeFn* out) {
+  static std::atomic<void*> cached{nullptr};
+  void* fn = cached.load();
+  if (!fn) {
+    cudaDriverEntryPointQueryResult q;
+    CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !fn) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled is not available");
+    cached.store(fn);
+  }
+  *out = (TensorMapEncodeFn)fn;
+  return RLXPP_OK;
+}
+
+// Opt-in shared memory of a kernel above the 48 KB default, set once per (kernel, device).
+template <class Kernel>
+static int allow_dynamic_smem(Kernel kernel, std::atomic<uint64_t>& done, int bytes) {
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 64 && (done.load() >> dev & 1)) return RLXPP_OK;
+  CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+  if (dev < 64) done.fetch_or(1ull << dev);
+  return RLXPP_OK;
 }
 
 // Tensor map of a stream-major output (UMMA engine, aligned): out[count][n_per] doubles viewed as
 // [count][n_per / 16][16], box 32 x 2 x 16, 128-byte swizzle (StreamMajorStage).  n_per >= 16.
-// cuTensorMapEncodeTiled comes from the driver through the runtime (no link against libcuda).
 static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count, uint64_t n_per, uint64_t pitch) {
-  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static EncodeFn encode = nullptr;
-  if (!encode) {
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
-    if (q != cudaDriverEntryPointSuccess || !fn) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled is not available");
-    encode = (EncodeFn)fn;
-  }
+  TensorMapEncodeFn encode = nullptr;
+  const int erc = tensor_map_encoder(&encode);
+  if (erc) return erc;
   if (n_per >= (1ull << 31) || count >= (1ull << 31))
     return fail(RLXPP_EINVAL, "stream-major output: n_per_stream and the stream count must be below 2^31");
   const cuuint64_t dims[3] = {16, n_per / 16, count};
@@ -1395,22 +1442,14 @@ static int encode_stream_major_map(CUtensorMap* map, double* out, uint64_t count
 // Tensor map of an interleaved float output (F32RowStage): float rows of `ld` floats, `count` of them written by this
 // launch, 2 n_per rows; box = 128 streams x 24 rows.  ld must be a multiple of 4 (16-byte row pitch).
 static int encode_f32_rows_map(CUtensorMap* map, float* out, uint64_t count, uint64_t ld, uint64_t rows) {
-  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static std::atomic<void*> cached{nullptr};
-  void* fn = cached.load();
-  if (!fn) {
-    cudaDriverEntryPointQueryResult q;
-    CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
-    if (q != cudaDriverEntryPointSuccess || !fn) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled is not available");
-    cached.store(fn);
-  }
+  TensorMapEncodeFn encode = nullptr;
+  const int erc = tensor_map_encoder(&encode);
+  if (erc) return erc;
   const cuuint64_t dims[2] = {count, rows};
   const cuuint64_t strides[1] = {ld * sizeof(float)};
   const cuuint32_t box[2] = {128, 24};
   const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = ((EncodeFn)fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr,
+  const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr,
                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled (float rows) failed (%d)", (int)r);
@@ -1442,23 +1481,11 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
   if (aligned) {
     constexpr bool kStaged = MODE == kStoreStreamMajor;  // the kernel's kStaged
-    if (kStaged) {  // 20 KB static + 33 KB of boxes: above the 48 KB default, 4 CTAs per SM still fit
+    // 20 KB static + 33 KB (stream-major boxes) or 36 KB (float-row boxes): above the 48 KB default, 4 CTAs per SM fit
+    if (kStaged || a.f32_boxes) {
       static std::atomic<uint64_t> done{0};  // one bit per device: function attributes are per device
-      int dev = 0;
-      CUDA_TRY(cudaGetDevice(&dev));
-      if (dev >= 64 || !(done.load() >> dev & 1)) {
-        CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)kStageCtaBytes));
-        CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                      cudaSharedmemCarveoutMaxShared));
-        if (dev < 64) done.fetch_or(1ull << dev);
-      }
-    }
-    if (a.f32_boxes) {  // 20 KB static + 36 KB of boxes: 4 CTAs per SM still fit
-      CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)kF32StageBytes));
-      CUDA_TRY(cudaFuncSetAttribute(tc_generate_kernel<MODE, true, OUT>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                    cudaSharedmemCarveoutMaxShared));
+      const int rc = allow_dynamic_smem(tc_generate_kernel<MODE, true, OUT>, done, (int)(kStaged ? kStageCtaBytes : kF32StageBytes));
+      if (rc) return rc;
     }
     tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, kStaged ? kStageCtaBytes : (a.f32_boxes ? kF32StageBytes : 0), s>>>(a);
   } else {
@@ -1517,6 +1544,23 @@ int rlxpp_set_chunks(int n_chunks) {
   return RLXPP_OK;
 }
 
+int rlxpp_rare_counts(uint64_t* out_host, int reset) {
+  static_assert(RLXPP_RARE_KINDS == kRareKinds, "rlxpp.h and arith.cuh disagree on the rare-path counters");
+  int rc = check_device();
+  if (rc) return rc;
+  CUDA_TRY(cudaDeviceSynchronize());
+  if (out_host) {
+    unsigned long long tmp[kRareKinds];
+    CUDA_TRY(cudaMemcpyFromSymbol(tmp, g_rare_counts, sizeof(tmp)));
+    for (int k = 0; k < kRareKinds; k++) out_host[k] = tmp[k];
+  }
+  if (reset) {
+    const unsigned long long zero[kRareKinds] = {};
+    CUDA_TRY(cudaMemcpyToSymbol(g_rare_counts, zero, sizeof(zero)));
+  }
+  return RLXPP_OK;
+}
+
 int rlxpp_has_fixed_multiplier(uint32_t p) {
 #define RLXPP_CASE(P) \
   if (p == P) return 1;
@@ -1558,7 +1602,7 @@ int rlxpp_create(rlxpp_t** hout, uint64_t n_streams, uint64_t seed, uint32_t p, 
   h->n = n_streams;
   h->p = p;
   h->stream = (cudaStream_t)cuda_stream;
-  build_tables(p, h->tables, true);
+  h->tables = cached_tables(p);
   h->fixed = fixed_level(p, h->tables.A);
   if (h->fixed < 0) {
     delete h;
@@ -1645,8 +1689,7 @@ int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, ui
   if ((uintptr_t)states_dev % 16) return fail(RLXPP_EINVAL, "rlxpp_advance_states: states must be 16-byte aligned");
   int rc = check_device();
   if (rc) return rc;
-  Tables t;
-  build_tables(p, t, false);
+  const Tables& t = cached_tables(p);
   const int fixed = fixed_level(p, t.A);
   if (fixed < 0) return fail(RLXPP_EINVAL, "rlxpp_advance_states: rows_generated.cuh is stale for p = %u", p);
   cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -1847,29 +1890,44 @@ int rlxpp_generate_doubles_host(rlxpp_t* h, double* out_host, uint64_t n_per_str
   if (rc) return rc;
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
   const int mode = layout == RLXPP_STREAM_MAJOR ? kStoreStreamMajor : kStoreInterleaved;
-  int buf = 0;
-  uint64_t done = 0;
-  for (uint64_t first = 0; first < h->n; first += chunk, buf ^= 1, done++) {
-    const uint64_t count = h->n - first < chunk ? h->n - first : chunk;
-    if (done >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copy[buf], 0));  // buffer free again
-    GenArgs a;
-    a.st = h->st; a.n_total = h->n; a.first = first; a.count = count; a.out = h->stage[buf]; a.ld = count;
-    a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
-    rc = launch_generate(h->fixed, a, mode, aligned, h->stream);
-    if (rc) return rc;
-    CUDA_TRY(cudaEventRecord(h->ev_kernel[buf], h->stream));
-    CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_kernel[buf], 0));
-    if (layout == RLXPP_STREAM_MAJOR) {
-      CUDA_TRY(cudaMemcpyAsync(out_host + first * n_per_stream, h->stage[buf], count * n_per_stream * sizeof(double),
-                               cudaMemcpyDeviceToHost, h->copy_stream));
-    } else {
-      CUDA_TRY(cudaMemcpy2DAsync(out_host + first, h->n * sizeof(double), h->stage[buf], count * sizeof(double),
-                                 count * sizeof(double), n_per_stream, cudaMemcpyDeviceToHost, h->copy_stream));
+  // A failure inside the loop leaves earlier stream ranges advanced and copies possibly in flight: drain both streams
+  // and stop trusting the cursor bookkeeping (the handle stays usable through the general path, or can be re-imported).
+  auto run = [&]() -> int {
+    int buf = 0;
+    uint64_t done = 0;
+    for (uint64_t first = 0; first < h->n; first += chunk, buf ^= 1, done++) {
+      const uint64_t count = h->n - first < chunk ? h->n - first : chunk;
+      if (done >= 2) CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_copy[buf], 0));  // buffer free again
+      GenArgs a;
+      a.st = h->st; a.n_total = h->n; a.first = first; a.count = count; a.out = h->stage[buf]; a.ld = count;
+      a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
+      const int lrc = launch_generate(h->fixed, a, mode, aligned, h->stream);
+      if (lrc) return lrc;
+      CUDA_TRY(cudaEventRecord(h->ev_kernel[buf], h->stream));
+      CUDA_TRY(cudaStreamWaitEvent(h->copy_stream, h->ev_kernel[buf], 0));
+      if (layout == RLXPP_STREAM_MAJOR) {
+        CUDA_TRY(cudaMemcpyAsync(out_host + first * n_per_stream, h->stage[buf], count * n_per_stream * sizeof(double),
+                                 cudaMemcpyDeviceToHost, h->copy_stream));
+      } else {
+        CUDA_TRY(cudaMemcpy2DAsync(out_host + first, h->n * sizeof(double), h->stage[buf], count * sizeof(double),
+                                   count * sizeof(double), n_per_stream, cudaMemcpyDeviceToHost, h->copy_stream));
+      }
+      CUDA_TRY(cudaEventRecord(h->ev_copy[buf], h->copy_stream));
     }
-    CUDA_TRY(cudaEventRecord(h->ev_copy[buf], h->copy_stream));
+    CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return RLXPP_OK;
+  };
+  rc = run();
+  if (rc) {
+    const std::string why = g_last_error;
+    cudaStreamSynchronize(h->copy_stream);
+    cudaStreamSynchronize(h->stream);
+    h->pos_uniform = false;
+    h->aligned = false;
+    g_last_error = why;
+    return rc;
   }
-  CUDA_TRY(cudaStreamSynchronize(h->copy_stream));
-  CUDA_TRY(cudaStreamSynchronize(h->stream));
   after_generate(h, n_per_stream);
   return RLXPP_OK;
 }
@@ -1973,11 +2031,13 @@ static int launch_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out, ui
   if (rc) return rc;
   const unsigned grid = grid_for(h->n);
   if (reduce) {
-    if (coop) ragged_kernel<true, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-    else ragged_kernel<false, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    if (coop == 2) ragged_kernel<2, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else if (coop) ragged_kernel<1, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else ragged_kernel<0, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
   } else {
-    if (coop) ragged_kernel<true, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-    else ragged_kernel<false, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    if (coop == 2) ragged_kernel<2, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else if (coop) ragged_kernel<1, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else ragged_kernel<0, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
   }
   LAUNCH_CHECK();
   return RLXPP_OK;

@@ -212,7 +212,10 @@ struct Tile {
 __device__ __forceinline__ void reduce_z(u32 (&z)[20], u32 (&x)[18]) {
   u32 rare = 0;
   fold_fast(z, x, rare);
-  if (__builtin_expect(rare != 0, 0)) mod_m20(z, x);  // inline: a call would force z, x into local memory
+  if (__builtin_expect(rare != 0, 0)) {
+    count_rare(fold_rare_mask(z[0], z[1], z[7], z[8], z[9], z[17], z[18], z[19]));
+    mod_m20(z, x);  // inline: a call would force z, x into local memory
+  }
 }
 
 }  // namespace tc

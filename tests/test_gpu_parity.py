@@ -461,12 +461,14 @@ def test_p24_floats_are_the_raw_ranlux_numbers(rlx, torch, oracle):
 
 
 # ------------------------------------------------------------------------------------- device API (8f-1)
-@pytest.mark.parametrize("coop", [True, False])
+@pytest.mark.parametrize("coop", [True, False, 2])
 def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, coop):
     """include/rlxpp_device.cuh through rlxpp_generate_ragged: every stream draws its own number of
     doubles (0 .. 70, so lanes of a warp run out of their blocks at different calls), from per-stream
     cursors, twice in a row, then the library's bulk kernel continues the same streams.  Everything
-    must be the one sequence the oracle gives for that stream; cooperative and per-thread advance agree."""
+    must be the one sequence the oracle gives for that stream; cooperative and per-thread advance agree,
+    and so does a kernel that alternates draw_coop() and draw() on the same Stream (coop = 2: a spare block
+    made by draw_coop() must be entered, not recomputed past, by draw())."""
     n, p, ld = 1000, 2048, 72
     dist = inputs.splitmix64(77, n) % np.uint64(30)
     c1 = (inputs.splitmix64(78, n) % np.uint64(71)).astype(np.uint32)
@@ -493,7 +495,7 @@ def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, 
     rlx.rlxpp_destroy(h)
 
 
-@pytest.mark.parametrize("coop", [True, False])
+@pytest.mark.parametrize("coop", [True, False, 2])
 def test_device_api_ragged_reduce(rlx, torch, oracle, nthreads, coop):
     n, p = 700, 389
     cnt = (inputs.splitmix64(5150, n) % np.uint64(200)).astype(np.uint32)
@@ -940,3 +942,47 @@ def test_interleaved_floats_through_row_boxes(rlx, torch, oracle, nthreads, bloc
         assert np.all(raw[2 * per * n:] == -1.0), "wrote behind the output buffer"
     check_state(rlx, torch, h, ref, "interleaved floats")
     rlx.rlxpp_destroy(h)
+
+
+# ------------------------------------------------------------------------------------- sharding
+def test_eight_shard_handles_reproduce_one_generator(rlx, torch, oracle, nthreads):
+    """The multi-GPU partition on one device, through librlxpp.so: a 2^13 + 37-stream job split into 8 contiguous ranges
+    (paper_2106_02504_b200/shard.py), one handle per range seeded with rank_seed(seed, first); the concatenation of the
+    shards' outputs (stream-major slabs, interleaved column blocks, fused sums, final states) is what ONE handle over
+    all streams gives, and what the oracle gives.  No collective: the ranks never exchange anything."""
+    from paper_2106_02504_b200 import shard
+    world, n_total, per, p, seed = 8, (1 << 13) + 37, 96, 2048, 2**64 - 4000  # seeds wrap mod 2^64 inside the job
+    one = rlx.rlxpp_create(n_total, seed, p)
+    whole_sm = torch.empty((n_total, per), dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_doubles(one, whole_sm, per, rlx.RLXPP_STREAM_MAJOR)
+    whole_s = torch.empty(n_total, dtype=torch.float64, device="cuda")
+    whole_q = torch.empty(n_total, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_reduce(one, whole_s, whole_q, 30)
+    sm = torch.full((n_total, per), -1.0, dtype=torch.float64, device="cuda")
+    il = torch.full((per, n_total), -1.0, dtype=torch.float64, device="cuda")
+    S = torch.full((n_total,), -1.0, dtype=torch.float64, device="cuda")
+    Q = torch.full((n_total,), -1.0, dtype=torch.float64, device="cuda")
+    handles = []
+    for r in range(world):
+        first, count = shard.stream_range(r, world, n_total)
+        h = rlx.rlxpp_create(count, shard.rank_seed(seed, first), p)
+        handles.append((h, first, count))
+        rlx.rlxpp_generate_doubles(h, sm[first:first + count], per, rlx.RLXPP_STREAM_MAJOR)  # its slab
+        rlx.rlxpp_generate_reduce(h, S[first:first + count], Q[first:first + count], 30)
+    torch.cuda.synchronize()
+    assert_bits_equal(sm.cpu().numpy(), whole_sm.cpu().numpy(), "8 shards vs one handle, stream-major")
+    assert_bits_equal(S.cpu().numpy(), whole_s.cpu().numpy(), "8 shards vs one handle, sums")
+    assert_bits_equal(Q.cpu().numpy(), whole_q.cpu().numpy(), "8 shards vs one handle, sums of squares")
+    # the interleaved column block of a rank is not contiguous in the job's array: each rank writes its own [per][count]
+    for h, first, count in handles:
+        blk = torch.empty((per, count), dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_doubles(h, blk, per, rlx.RLXPP_INTERLEAVED)
+        il[:, first:first + count] = blk
+    ref = oracle.streams(inputs.seeds(n_total, seed), p, per + 30 + per, want=("doubles", "state"), nthreads=nthreads)
+    assert_bits_equal(sm.cpu().numpy(), ref["doubles"][:, :per], "8 shards vs oracle")
+    assert_bits_equal(il.cpu().numpy().T, ref["doubles"][:, per + 30:], "8 shards vs oracle, interleaved blocks")
+    for h, first, count in handles:
+        sub = {k: v[first:first + count] for k, v in ref.items()}
+        check_state(rlx, torch, h, sub, f"shard starting at stream {first}")
+        rlx.rlxpp_destroy(h)
+    rlx.rlxpp_destroy(one)

@@ -137,6 +137,35 @@ def test_public_device_header_is_self_contained(tmp_path):
     assert res.returncode == 0, res.stdout + res.stderr
 
 
+def test_fixed_multiplier_rows_header_is_what_its_generator_writes(tmp_path):
+    """csrc/rows_generated.cuh (the IMAD engine's 4 x 324 immediates) is committed although build() regenerates it;
+    it must be exactly csrc/gen_rows.py's output, and its immediates must be the limbs of A 2^(32 i) mod m."""
+    import importlib.util
+    import re
+    here = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2106_02504_b200", "csrc")
+    spec = importlib.util.spec_from_file_location("gen_rows", os.path.join(here, "gen_rows.py"))
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
+    tracked = open(os.path.join(here, "rows_generated.cuh")).read()
+    body = "\n\n".join(gen.emit_level(p) for p in gen.LEVELS)
+    assert body in tracked, "rows_generated.cuh is stale: run python -m paper_2106_02504_b200.build"
+    # the immediates themselves, against Python: row i of level p = limbs of a^p 2^(32 i) mod m (324 per level)
+    for p, block in zip(gen.LEVELS, re.split(r"// ---- p = \d+:", tracked)[1:]):
+        A = pow(A1, p, M)
+        kA = [int(v, 16) for v in re.findall(r"0x([0-9a-f]{8})u", block.split("kA[18]")[1].split(";")[0])]
+        assert sum(v << (32 * i) for i, v in enumerate(kA)) == A
+        row0 = [int(v, 16) for v in re.findall(r"x\[0\] \* 0x([0-9a-f]{8})u", block)]
+        assert len(row0) == 18
+        rows = {0: [row0[2 * (k // 2) + (k % 2)] for k in range(18)]}  # E[k], O[k] pairs are columns 2k, 2k + 1
+        for i, asm in enumerate(re.findall(r"// row (\d+)\n(.*?)\"}\"", block, re.S)):
+            imm = [int(v, 16) for v in re.findall(r"%20, 0x([0-9a-f]{8});", asm[1])]
+            assert len(imm) == 18 and int(asm[0]) == i + 1
+            rows[i + 1] = [imm[k // 2] if k % 2 == 0 else imm[9 + k // 2] for k in range(18)]  # even chain, then odd chain
+        assert len(rows) == 18
+        for i in range(18):
+            assert sum(v << (32 * k) for k, v in enumerate(rows[i])) == (A << (32 * i)) % M, (p, i)
+
+
 def test_normal_coefficients_header_is_what_its_generator_writes():
     """csrc/normal_coeffs.cuh (polynomials of rlxpp_generate_normal) is committed; it must be the output of
     csrc/gen_normal_coeffs.py (mpmath near-minimax fits), and the fits must be as good as the header says."""

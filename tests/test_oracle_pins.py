@@ -464,6 +464,11 @@ def test_splitmix64_and_cfg2_inputs(oracle):
     A16 = pow(A1, 2048 * 16, M)
     for i in list(range(0, 256, 17)) + list(range(256, 320)):
         assert inputs.limbs_to_int(out[i]) == A16 * inputs.limbs_to_int(st[i]) % M
+    # reps == 0 only canonicalises (its own branch in orc_advance_states): Python's % on every edge state, incl. [m, 2^576)
+    out0 = oracle.advance_states(st, 2048, 0)
+    for i in range(320):
+        assert inputs.limbs_to_int(out0[i]) == inputs.limbs_to_int(st[i]) % M
+    assert any(inputs.limbs_to_int(s) >= M for s in st[256:])
 
 
 # ----------------------------------------------------------------- normals (DESIGN reading N-1)

@@ -68,3 +68,46 @@ def test_two_gloo_ranks_reproduce_one_generator(tmp_path, oracle):
     assert whole.shape == ref.shape
     assert np.array_equal(whole.view(np.uint64), ref.view(np.uint64))
     assert float(np.load(tmp_path / "slowest.npy")[0]) == 11.0  # max over ranks of 10 + rank
+
+
+def test_bench_rank_logic_for_eight_ranks():
+    """bench.py --gpus 8 on the host side (the pool has one GPU per lease: no scaling curve is measured).  Weak scaling:
+    every rank owns its own 2^20 streams, the ranges tile the 8 x 2^20-stream job, rank g's seed argument is the job's
+    seed + its first stream, and `value` is all ranks' units over the slowest rank's time."""
+    import bench
+    world, per_gpu = 8, 1 << 20
+    lay = [bench.job_layout(r, world, per_gpu) for r in range(world)]
+    assert [f for f, _, _ in lay] == [r * per_gpu for r in range(world)]
+    assert all(c == per_gpu for _, c, _ in lay)
+    assert [s for _, _, s in lay] == [1 + r * per_gpu for r in range(world)]  # seeds 1 .. 8 x 2^20, no overlap, no gap
+    assert bench.job_layout(3, 8, 1 << 20, seed=2**64 - 5)[2] == (2**64 - 5 + 3 * (1 << 20)) % 2**64
+    units = per_gpu * 1536
+    assert bench.whole_job_rate(units, world, 2.0) == 8 * units / 2e-3
+    assert bench.whole_job_rate(units, 1, 2.0) * 8 == bench.whole_job_rate(units, 8, 2.0)  # 100 % weak scaling = 8 x
+    sp = bench.spread([3.0, 1.0, 2.0, 10.0])
+    assert (sp["min"], sp["median"], sp["max"], sp["n"]) == (1.0, 2.5, 10.0, 4)
+
+
+def _max_worker(rank, world, port, tmpdir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        slowest = shard.max_over_ranks(2.0 + 0.125 * ((rank * 5) % world), dist)
+        if rank == world - 1:
+            np.save(os.path.join(tmpdir, "slowest8.npy"), np.array([slowest]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_eight_gloo_ranks_agree_on_the_slowest():
+    """The only communication of the multi-GPU bench: the job's time is the MAX over ranks (here 8 gloo ranks)."""
+    import tempfile
+    import torch.multiprocessing as mp
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    with tempfile.TemporaryDirectory() as d:
+        mp.spawn(_max_worker, args=(8, port, d), nprocs=8, join=True)
+        assert float(np.load(os.path.join(d, "slowest8.npy"))[0]) == 2.0 + 0.125 * 7
