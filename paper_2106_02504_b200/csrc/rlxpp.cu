@@ -991,6 +991,196 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_k
   tile.teardown();
 }
 
+// Fused sum / sum of squares (S8 a-7b, cfg5) with TWO tiles per CTA on one accumulator (tc::PairTile): nothing is
+// stored, so the kernel is a chain of advances per tile, and interleaving two chains hides the tensor pipe's round
+// trip behind the other tile's integer work.  Work item = (PAIR of adjacent tiles, chunk of draws); n_tiles counts pairs.
+// Same contract and the same per-stream arithmetic as tc_generate_kernel<kReduce, ...>.
+#ifndef RLXPP_PAIR_SYNC
+#define RLXPP_PAIR_SYNC tc::kSyncCta
+#endif
+template <bool ALIGNED>
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kernel(const __grid_constant__ GenArgs a) {
+  __shared__ tc::PairSmem smem;
+  tc::PairTile<RLXPP_PAIR_SYNC> tile;
+  tile.setup(smem, a.bmat);
+  const u32 kexp = a.kexp;
+  const u64 n_items = (u64)a.n_tiles * a.n_chunks;
+  for (;;) {
+    if (threadIdx.x == 0) smem.ticket = atomicAdd(a.sched, 1u);
+    __syncthreads();
+    const u64 w = smem.ticket;
+    if (w >= n_items) break;
+    const u32 pidx = (u32)(w % a.n_tiles), chunk = (u32)(w / a.n_tiles);
+    if (chunk > 0) {
+      if (threadIdx.x == 0) {
+        u32 done;
+        do {
+          asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(a.sched + 1 + pidx) : "memory");
+        } while (done < chunk);
+      }
+      __syncthreads();
+    }
+    const u64 t0 = (u64)chunk * a.chunk_len;
+    const u64 n = a.n_per - t0 < a.chunk_len ? a.n_per - t0 : a.chunk_len;
+    const u64 smax = n ? (12 + (n - 1)) / 12 : 0;  // unaligned: last block of any thread (uniform)
+    u64 il[2];
+    bool live[2], early[2];
+    u32 pos[2], newpos[2];
+    Sink<kReduce> sink[2];
+    u32 x[18], v[18], c;
+#pragma unroll
+    for (int t = 0; t < 2; t++) {
+      il[t] = ((u64)pidx * 2 + t) * tc::kTile + threadIdx.x;
+      live[t] = il[t] < a.count;
+      pos[t] = 12;
+#pragma unroll
+      for (int j = 0; j < 18; j++) x[j] = 0;
+      if (live[t]) load_state(a.st, a.n_total, a.first + il[t], x, pos[t]);
+      sink[t].p = nullptr;
+      sink[t].ld = 0;
+      sink[t].kexp = kexp;
+      sink[t].S = 0.0;
+      sink[t].Q = 0.0;
+      if (chunk > 0 && live[t]) {
+        sink[t].S = __ldcg(a.sum + il[t]);
+        sink[t].Q = __ldcg(a.sumsq + il[t]);
+      }
+      const u64 last = n ? ((u64)pos[t] + (n - 1)) / 12 : 0;  // own last block
+      early[t] = last < smax;
+      newpos[t] = (u32)((u64)pos[t] + n - 12 * last);
+      if (!ALIGNED && n > 0 && pos[t] < 12) {  // block 0 = the current block
+        to_ranlux_exact(x, v, c);
+        if (live[t]) EmitBlock<0, kReduce>::masked(sink[t], v, 0, pos[t], n);
+      }
+      tile.stash(t, x);
+    }
+    if (ALIGNED) {
+      const u64 nblk = n / 12;
+      if (nblk > 0) tile.start(0);
+#pragma unroll 1
+      for (u64 b = 0; b < nblk; b++) {
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+          u32 cols[72], z[20];
+          tile.load(cols);
+          if (t == 0 || b + 1 < nblk) tile.start(t ^ 1);  // the other tile's MMA runs under this tile's integer work
+          tc::normalise(cols, z);
+          tc::reduce_z(z, x);
+          if (b + 1 < nblk) tile.stash(t, x);
+          else if (live[t]) store_state(a.st, a.n_total, a.first + il[t], x, 12u);
+          to_ranlux_hot(x, v, c);
+          if (live[t]) EmitBlock<0, kReduce>::all(sink[t], v, 0);
+        }
+      }
+    } else if (n > 0) {
+      tile.start(0);
+      // blocks 1 .. smax - 2 lie wholly inside [0, n) for every cursor: no masks
+      u64 s = 1;
+#pragma unroll 1
+      for (; s + 2 <= smax; s++) {
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+          u32 cols[72], z[20];
+          tile.load(cols);
+          tile.start(t ^ 1);
+          tc::normalise(cols, z);
+          tc::reduce_z(z, x);
+          tile.stash(t, x);
+          to_ranlux_hot(x, v, c);
+          if (live[t]) EmitBlock<0, kReduce>::template all<false>(sink[t], v, 0);
+        }
+      }
+      // the last two blocks carry per-draw masks; a stream that ends one block early (early[t]) discards the last
+      // product.  Every stream takes block smax - 1 (if there is one), so the state is written there and again at smax.
+#pragma unroll 1
+      for (; s <= smax; s++) {
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+          u32 cols[72], z[20];
+          tile.load(cols);
+          if (t == 0 || s < smax) tile.start(t ^ 1);
+          tc::normalise(cols, z);
+          tc::reduce_z(z, x);
+          if (s < smax) tile.stash(t, x);
+          if (!(s == smax && early[t])) {
+            if (live[t]) store_state(a.st, a.n_total, a.first + il[t], x, newpos[t]);
+            to_ranlux_hot(x, v, c);
+            if (live[t]) EmitBlock<0, kReduce>::masked(sink[t], v, s * 12, pos[t], n);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < 2; t++) {
+      if (!live[t]) continue;
+      if (!ALIGNED && n > 0 && smax == 1 && early[t]) {  // never advanced: only the cursor moves
+        uint4 q = __ldcg(a.st + 4 * a.n_total + a.first + il[t]);
+        q.z = newpos[t];
+        a.st[4 * a.n_total + a.first + il[t]] = q;
+      }
+      a.sum[il[t]] = sink[t].S;
+      if (a.sumsq) a.sumsq[il[t]] = sink[t].Q;
+    }
+    if (a.n_chunks > 1) {  // publish: state and partial sums of this pair are in global memory
+      __threadfence();
+      __syncthreads();
+      if (threadIdx.x == 0)
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.sched + 1 + pidx), "r"(chunk + 1u) : "memory");
+    } else {
+      __syncthreads();  // smem.ticket is rewritten at the top of the loop
+    }
+  }
+  tile.teardown();
+}
+
+// Raw advance (cfg2) with two tiles per CTA on one accumulator; one CTA per pair of tiles.
+template <int LAYOUT>
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_pair_kernel(u64* __restrict__ states, u64 n, u32 reps,
+                                                                                         const uint4* __restrict__ bmat) {
+  __shared__ tc::PairSmem smem;
+  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kRawStageWords : 1];
+  tc::PairTile<tc::kSyncArrive> tile;
+  tile.setup(smem, bmat);
+  const u64 n_tiles = (n + kThreads - 1) / kThreads, n_pairs = (n_tiles + 1) / 2;
+#pragma unroll 1
+  for (u64 pair = blockIdx.x; pair < n_pairs; pair += gridDim.x) {
+    u32 x[18];
+#pragma unroll
+    for (int t = 0; t < 2; t++) {
+      const u64 blk = 2 * pair + t;
+#pragma unroll
+      for (int j = 0; j < 18; j++) x[j] = 0;
+      if (blk < n_tiles) {  // uniform
+        load_raw<LAYOUT>(states, n, stage, x, blk);
+        if (reps == 0) {
+          canonicalise(x);
+          store_raw<LAYOUT>(states, n, stage, x, blk);
+        }
+        __syncthreads();  // the staging buffer is reused
+      }
+      tile.stash(t, x);
+    }
+    if (reps > 0) tile.start(0);
+#pragma unroll 1
+    for (u32 r = 0; r < reps; r++) {
+#pragma unroll
+      for (int t = 0; t < 2; t++) {
+        u32 cols[72], z[20];
+        tile.load(cols);
+        if (t == 0 || r + 1 < reps) tile.start(t ^ 1);
+        tc::normalise(cols, z);
+        tc::reduce_z(z, x);
+        if (r + 1 < reps) tile.stash(t, x);
+        else if (2 * pair + t < n_tiles) {
+          store_raw<LAYOUT>(states, n, stage, x, 2 * pair + t);
+          __syncthreads();
+        }
+      }
+    }
+  }
+  tile.teardown();
+}
+
 // Seeding and skip-ahead ("fast exponentiation by squaring"): x <- x * prod_b T[b]^(bit b of e)
 // with T[b] = base^(2^b) precomputed on the host (64 entries of 18 limbs).  A bit is processed by
 // the whole warp if any lane has it set; lanes without it keep their value.
@@ -1467,7 +1657,8 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per, a.pitch ? a.pitch : a.n_per);
     if (rc) return rc;
   }
-  const uint64_t n_tiles = (a.count + tc::kTile - 1) / tc::kTile;
+  // the fused reduce runs two tiles per CTA (tc_reduce_pair_kernel): its work items are pairs of tiles
+  const uint64_t n_tiles = MODE == kReduce ? (a.count + 2 * tc::kTile - 1) / (2 * tc::kTile) : (a.count + tc::kTile - 1) / tc::kTile;
   const unsigned slots = tc_slots();
   a.n_tiles = (u32)n_tiles;
   plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len);
@@ -1479,7 +1670,10 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   const uint64_t items = n_tiles * a.n_chunks;
   const unsigned grid = (unsigned)(items < slots ? items : slots);
   CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
-  if (aligned) {
+  if (MODE == kReduce) {
+    if (aligned) tc_reduce_pair_kernel<true><<<grid, tc::kTile, 0, s>>>(a);
+    else tc_reduce_pair_kernel<false><<<grid, tc::kTile, 0, s>>>(a);
+  } else if (aligned) {
     constexpr bool kStaged = MODE == kStoreStreamMajor;  // the kernel's kStaged
     // 20 KB static + 33 KB (stream-major boxes) or 36 KB (float-row boxes): above the 48 KB default, 4 CTAs per SM fit
     if (kStaged || a.f32_boxes) {
@@ -1701,9 +1895,10 @@ int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, ui
     // one CTA per tile: measured faster than a persistent grid here (1,050 vs 946 G doubles-equivalent/s at
     // cfg2: with 16 advances per tile the load / compute / store phases of co-resident CTAs overlap better when
     // the CTAs are not in lock step); the kernel's tile loop serves grids smaller than the tile count
-    const unsigned grid = (unsigned)(tiles < (1u << 30) ? tiles : (1u << 30));
-    if (layout == RLXPP_AOS) tc_advance_states_kernel<RLXPP_AOS><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
-    else tc_advance_states_kernel<RLXPP_SOA><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
+    const uint64_t pairs = (tiles + 1) / 2;  // two tiles per CTA on one accumulator (tc::PairTile)
+    const unsigned grid = (unsigned)(pairs < (1u << 30) ? pairs : (1u << 30));
+    if (layout == RLXPP_AOS) tc_advance_states_pair_kernel<RLXPP_AOS><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
+    else tc_advance_states_pair_kernel<RLXPP_SOA><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
     LAUNCH_CHECK();
     return RLXPP_OK;
   }

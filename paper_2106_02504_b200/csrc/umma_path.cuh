@@ -68,6 +68,50 @@ struct Smem {
   u32 ticket;                  // work item of the persistent scheduler (rlxpp.cu)
 };
 
+// The 72 accumulator columns of one stream -> Z = sum_n acc_n 2^(8n) as 19 limbs (z[18] < 2^15, z[19] = 0).
+__device__ __forceinline__ void normalise(const u32 (&c)[72], u32 (&z)[20]) {
+  // limb k gets columns 4k .. 4k+3 at byte offsets 0, 8, 16, 24.  e_k = c0 + (c1 << 8) and
+  // o_k = c2 + (c3 << 8) are both < 2^23 + 2^31 < 2^32, so  Z = E + (O << 16)  with E, O the
+  // 18-limb numbers of limbs e_k, o_k: 36 shift-adds, 19 byte permutes, one 19-limb carry chain.
+  u32 e[18], o[18], t[19];
+#pragma unroll
+  for (int k = 0; k < 18; k++) {
+    e[k] = c[4 * k] + (c[4 * k + 1] << 8);
+    o[k] = c[4 * k + 2] + (c[4 * k + 3] << 8);
+  }
+  t[0] = o[0] << 16;
+#pragma unroll
+  for (int k = 1; k < 18; k++) t[k] = __byte_perm(o[k - 1], o[k], 0x5432);
+  t[18] = o[17] >> 16;
+  asm("add.cc.u32 %0, %19, %37;\n\t"
+      "addc.cc.u32 %1, %20, %38;\n\t"
+      "addc.cc.u32 %2, %21, %39;\n\t"
+      "addc.cc.u32 %3, %22, %40;\n\t"
+      "addc.cc.u32 %4, %23, %41;\n\t"
+      "addc.cc.u32 %5, %24, %42;\n\t"
+      "addc.cc.u32 %6, %25, %43;\n\t"
+      "addc.cc.u32 %7, %26, %44;\n\t"
+      "addc.cc.u32 %8, %27, %45;\n\t"
+      "addc.cc.u32 %9, %28, %46;\n\t"
+      "addc.cc.u32 %10, %29, %47;\n\t"
+      "addc.cc.u32 %11, %30, %48;\n\t"
+      "addc.cc.u32 %12, %31, %49;\n\t"
+      "addc.cc.u32 %13, %32, %50;\n\t"
+      "addc.cc.u32 %14, %33, %51;\n\t"
+      "addc.cc.u32 %15, %34, %52;\n\t"
+      "addc.cc.u32 %16, %35, %53;\n\t"
+      "addc.cc.u32 %17, %36, %54;\n\t"
+      "addc.u32 %18, %55, 0;"
+      : "=r"(z[0]), "=r"(z[1]), "=r"(z[2]), "=r"(z[3]), "=r"(z[4]), "=r"(z[5]), "=r"(z[6]), "=r"(z[7]), "=r"(z[8]),
+        "=r"(z[9]), "=r"(z[10]), "=r"(z[11]), "=r"(z[12]), "=r"(z[13]), "=r"(z[14]), "=r"(z[15]), "=r"(z[16]),
+        "=r"(z[17]), "=r"(z[18])
+      : "r"(e[0]), "r"(e[1]), "r"(e[2]), "r"(e[3]), "r"(e[4]), "r"(e[5]), "r"(e[6]), "r"(e[7]), "r"(e[8]), "r"(e[9]),
+        "r"(e[10]), "r"(e[11]), "r"(e[12]), "r"(e[13]), "r"(e[14]), "r"(e[15]), "r"(e[16]), "r"(e[17]), "r"(t[0]),
+        "r"(t[1]), "r"(t[2]), "r"(t[3]), "r"(t[4]), "r"(t[5]), "r"(t[6]), "r"(t[7]), "r"(t[8]), "r"(t[9]), "r"(t[10]),
+        "r"(t[11]), "r"(t[12]), "r"(t[13]), "r"(t[14]), "r"(t[15]), "r"(t[16]), "r"(t[17]), "r"(t[18]));
+  z[19] = 0;
+}
+
 template <int SYNC>
 struct Tile {
   u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of the A tile
@@ -158,49 +202,124 @@ struct Tile {
     umma::fence_after_sync();
     u32 c[72];
     umma::tmem_ld72_wait(tld, tld + 64u, c);
-    // limb k gets columns 4k .. 4k+3 at byte offsets 0, 8, 16, 24.  e_k = c0 + (c1 << 8) and
-    // o_k = c2 + (c3 << 8) are both < 2^23 + 2^31 < 2^32, so  Z = E + (O << 16)  with E, O the
-    // 18-limb numbers of limbs e_k, o_k: 36 shift-adds, 19 byte permutes, one 19-limb carry chain.
-    u32 e[18], o[18], t[19];
-#pragma unroll
-    for (int k = 0; k < 18; k++) {
-      e[k] = c[4 * k] + (c[4 * k + 1] << 8);
-      o[k] = c[4 * k + 2] + (c[4 * k + 3] << 8);
-    }
-    t[0] = o[0] << 16;
-#pragma unroll
-    for (int k = 1; k < 18; k++) t[k] = __byte_perm(o[k - 1], o[k], 0x5432);
-    t[18] = o[17] >> 16;
-    asm("add.cc.u32 %0, %19, %37;\n\t"
-        "addc.cc.u32 %1, %20, %38;\n\t"
-        "addc.cc.u32 %2, %21, %39;\n\t"
-        "addc.cc.u32 %3, %22, %40;\n\t"
-        "addc.cc.u32 %4, %23, %41;\n\t"
-        "addc.cc.u32 %5, %24, %42;\n\t"
-        "addc.cc.u32 %6, %25, %43;\n\t"
-        "addc.cc.u32 %7, %26, %44;\n\t"
-        "addc.cc.u32 %8, %27, %45;\n\t"
-        "addc.cc.u32 %9, %28, %46;\n\t"
-        "addc.cc.u32 %10, %29, %47;\n\t"
-        "addc.cc.u32 %11, %30, %48;\n\t"
-        "addc.cc.u32 %12, %31, %49;\n\t"
-        "addc.cc.u32 %13, %32, %50;\n\t"
-        "addc.cc.u32 %14, %33, %51;\n\t"
-        "addc.cc.u32 %15, %34, %52;\n\t"
-        "addc.cc.u32 %16, %35, %53;\n\t"
-        "addc.cc.u32 %17, %36, %54;\n\t"
-        "addc.u32 %18, %55, 0;"
-        : "=r"(z[0]), "=r"(z[1]), "=r"(z[2]), "=r"(z[3]), "=r"(z[4]), "=r"(z[5]), "=r"(z[6]), "=r"(z[7]), "=r"(z[8]),
-          "=r"(z[9]), "=r"(z[10]), "=r"(z[11]), "=r"(z[12]), "=r"(z[13]), "=r"(z[14]), "=r"(z[15]), "=r"(z[16]),
-          "=r"(z[17]), "=r"(z[18])
-        : "r"(e[0]), "r"(e[1]), "r"(e[2]), "r"(e[3]), "r"(e[4]), "r"(e[5]), "r"(e[6]), "r"(e[7]), "r"(e[8]), "r"(e[9]),
-          "r"(e[10]), "r"(e[11]), "r"(e[12]), "r"(e[13]), "r"(e[14]), "r"(e[15]), "r"(e[16]), "r"(e[17]), "r"(t[0]),
-          "r"(t[1]), "r"(t[2]), "r"(t[3]), "r"(t[4]), "r"(t[5]), "r"(t[6]), "r"(t[7]), "r"(t[8]), "r"(t[9]), "r"(t[10]),
-          "r"(t[11]), "r"(t[12]), "r"(t[13]), "r"(t[14]), "r"(t[15]), "r"(t[16]), "r"(t[17]), "r"(t[18]));
-    z[19] = 0;
+    normalise(c, z);
   }
 
   // CTA-collective, after the last collect().
+  __device__ __forceinline__ void teardown() {
+    umma::fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) umma::tmem_dealloc(tmem, kTmemCols);
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// Two tiles per CTA on ONE accumulator (the kernels no store path binds: fused reduce, raw advance).
+// A tile's advances are a serial chain  MMA -> tcgen05.ld -> normalise + fold -> A-tile store -> MMA ..., and with one
+// tile per CTA the threads sit idle for the MMA + commit + mbarrier round trip of every advance; TMEM (4 x 128
+// allocated columns) caps the SM at four such chains.  The accumulator, however, is only live between the MMA and
+// the tcgen05.ld that empties it into registers.  So a CTA of 128 threads owns TWO tiles (thread r = stream r of
+// both), each with its own A tile in shared memory, sharing the 80 accumulator columns in time:
+//
+//     load(t):   wait for MMA(t)  ->  tcgen05.ld + wait::ld                  (accumulator now free)
+//     start(t'): hand-off barrier ->  issuing thread: MMA(t') + commit       (t' = the other tile; its A tile was
+//                                                                             stored in the previous half-step)
+//     normalise + fold tile t, stash(t) its new state for the next MMA(t), convert and consume its block
+//
+// MMA(t') runs under the ~250 instructions per warp of tile t's integer work: 8 chains per SM with the same 16 warps,
+// same TMEM, and no thread ever waits for the tensor pipe's round trip.  Ordering: every thread's tcgen05.ld of
+// the accumulator is complete (wait::ld, fence::before_thread_sync) before the hand-off barrier that precedes the next
+// MMA; MMA(t)'s reads of A tile t are complete (mbarrier) before stash(t) overwrites it; one mbarrier serves both
+// tiles because at most one commit is ever outstanding.
+struct PairSmem {
+  __align__(128) uint8_t a[2][kABytes];
+  __align__(128) uint8_t b[kBBytes];
+  __align__(8) u64 bar;
+  u32 tmem_slot;
+  u32 ticket;
+};
+
+template <int SYNC>
+struct PairTile {
+  u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of A tile 0 (tile 1: + kABytes)
+  u32 bar, phase, tmem, tld, issuer;
+  u64 adesc, bdesc;  // adesc: A tile 0
+
+  __device__ __forceinline__ void setup(PairSmem& s, const uint4* __restrict__ bmat) {
+    const u32 tid = threadIdx.x;
+    uint4* sb = reinterpret_cast<uint4*>(s.b);
+    for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
+    a_row = umma::smem_u32(s.a[0]) + tid * 16u;
+#pragma unroll
+    for (u32 t = 0; t < 2; t++)  // K bytes 80..95 of every row stay zero for the whole kernel
+      asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a_row + t * kABytes + 5u * kAChunk), "r"(0u) : "memory");
+    bar = umma::smem_u32(&s.bar);
+    phase = 0;
+    if (tid == 0) {
+      umma::mbar_init(bar, 1);
+      umma::fence_mbar_init();
+    }
+    if (tid < 32) {
+      umma::tmem_alloc(umma::smem_u32(&s.tmem_slot), kTmemCols);
+      umma::tmem_relinquish();
+    }
+    umma::fence_before_sync();
+    __syncthreads();
+    umma::fence_after_sync();
+    tmem = *reinterpret_cast<volatile u32*>(&s.tmem_slot);
+    issuer = SYNC == kSyncArrive ? ((tmem & 0xFFFFu) / kTmemCols) & 3u : 0u;
+    tld = tmem + (((tid >> 5) & 3u) << 21);
+    adesc = umma::smem_desc(umma::smem_u32(s.a[0]), kAChunk, 128u);
+    bdesc = umma::smem_desc(umma::smem_u32(s.b), kBChunk, 128u);
+  }
+
+  // this thread's state of tile t -> A tile t (any value < 2^576), visible to the tensor core after the next start(t)
+  __device__ __forceinline__ void stash(u32 t, const u32 (&x)[18]) {
+    const u32 row = a_row + t * kABytes;
+#pragma unroll
+    for (int g = 0; g < 4; g++)
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(row + (u32)g * kAChunk), "r"(x[4 * g]), "r"(x[4 * g + 1]),
+                   "r"(x[4 * g + 2]), "r"(x[4 * g + 3])
+                   : "memory");
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(row + 4u * kAChunk), "r"(x[16]), "r"(x[17]), "r"(0u) : "memory");
+    umma::fence_proxy_async_smem();
+  }
+
+  // CTA-collective: every thread has stashed tile t and emptied the accumulator; D = Xbytes(t) * B^T starts
+  __device__ __forceinline__ void start(u32 t) {
+    umma::fence_before_sync();
+    if (SYNC == kSyncArrive) {
+      if ((threadIdx.x >> 5) == issuer) {
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (umma::elect_one()) issue_mma(t);
+        __syncwarp();
+      } else {
+        asm volatile("bar.arrive 1, 128;" ::: "memory");
+      }
+    } else {
+      __syncthreads();
+      if (threadIdx.x == 0) issue_mma(t);
+      __syncwarp();
+    }
+  }
+  __device__ __forceinline__ void issue_mma(u32 t) {
+    umma::fence_after_sync();
+    const u64 ad = adesc + (u64)((t * kABytes) >> 4);
+#pragma unroll
+    for (u32 k = 0; k < 3; k++)
+      umma::mma_i8(tmem, ad + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
+    umma::commit(bar);
+  }
+
+  // waits for the MMA in flight and empties the accumulator into this thread's registers
+  __device__ __forceinline__ void load(u32 (&c)[72]) {
+    umma::mbar_wait(bar, phase);
+    phase ^= 1u;
+    __syncwarp();
+    umma::fence_after_sync();
+    umma::tmem_ld72_wait(tld, tld + 64u, c);
+  }
+
   __device__ __forceinline__ void teardown() {
     umma::fence_before_sync();
     __syncthreads();
