@@ -270,6 +270,12 @@ struct GenArgs {
   u32 n_tiles, n_chunks;
   u64 chunk_len;      // draws per chunk (a multiple of 96 = 8 blocks when n_chunks > 1)
   u32 kexp = kExp16;  // see arith.cuh: a launch parameter on purpose
+  // time-parallel path of short calls (tc_generate_lanes_kernel): images of the byte matrices of A^1 .. A^kMaxLanes,
+  // lanes per tile, and one reader counter per tile
+  const uint4* bmat_pow = nullptr;
+  u32 lanes = 0;
+  u32* lane_sync = nullptr;
+  u32 p = 0;  // luxury level (selects the cached matrices)
   // UMMA engine, aligned stream-major stores: tensor map of out (StreamMajorStage)
   alignas(64) CUtensorMap tmap;
 };
@@ -991,6 +997,73 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_k
   tile.teardown();
 }
 
+// Short calls (cfg1: 8 tiles x 32 blocks, S8d "launch-latency dominated"): a tile's blocks are a serial chain only if
+// they are computed one from the other.  Block b of a stream is to_ranlux(A^(b+1) X) (D7; "fast exponentiation"),
+// so with the byte matrices of A^1 .. A^K at hand, K CTAs ("lanes") work on ONE tile at once: lane j reads the stored
+// state, reaches block j with ONE pass against the matrix of A^(j+1), and then strides through blocks j + K, j + 2K, ...
+// with the matrix of A^K.  cfg1 becomes 256 CTAs of one pass each instead of 8 CTAs of 32 passes.  The lane that
+// computes the last block holds A^nblk X = the new state; it writes it in place once all K lanes of the tile have
+// read the old one (one counter per tile, left at zero again; all CTAs of the grid are co-resident by construction).
+// Aligned cursors, whole blocks, every store mode and output form (direct stores: the outputs are L2-sized).
+constexpr u32 kMaxLanes = 32;
+template <int MODE, int OUT>
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_lanes_kernel(const __grid_constant__ GenArgs a) {
+  static_assert(MODE != kReduce, "the fused sums are sequential in the draw index");
+  __shared__ tc::Smem smem;
+  __shared__ __align__(128) uint8_t bstride[tc::kBBytes];  // matrix of A^lanes: every pass after a lane's first
+  const u32 K = a.lanes, tidx = blockIdx.x / K, lane = blockIdx.x % K;
+  const u64 nblk = a.n_per / 12;
+  const bool strides = lane + K < nblk;  // this lane makes more than one pass
+  if (strides) {
+    const uint4* src = a.bmat_pow + (u64)(K - 1) * (tc::kBBytes / 16);
+    uint4* dst = reinterpret_cast<uint4*>(bstride);
+    for (u32 q = threadIdx.x; q < tc::kBBytes / 16; q += tc::kTile) dst[q] = __ldg(src + q);
+  }
+  tc::Tile<tc::kSyncCta> tile;
+  tile.setup(smem, a.bmat_pow + (u64)lane * (tc::kBBytes / 16));  // the matrix of A^(lane + 1)
+  const u64 il = (u64)tidx * tc::kTile + threadIdx.x;
+  const bool live = il < a.count;
+  u32 x[18], v[18], pos = 12, c;
+#pragma unroll
+  for (int j = 0; j < 18; j++) x[j] = 0;
+  if (live) load_state(a.st, a.n_total, a.first + il, x, pos);
+  Sink<MODE, OUT> sink;
+  sink.ld = a.ld;
+  sink.S = 0.0;
+  sink.Q = 0.0;
+  sink.kexp = kExp16;
+  if (MODE == kStoreStreamMajor) sink.p = a.out + il * (a.pitch ? a.pitch : a.n_per);
+  else if (OUT == kF32) sink.p = reinterpret_cast<double*>(reinterpret_cast<float*>(a.out) + il);
+  else sink.p = a.out + il;
+  tile.issue(x);  // (CTA barrier inside: every thread's state now sits in shared memory)
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(a.lane_sync + tidx, 1u);  // this lane has read the tile's state
+  }
+  if (strides) tile.bdesc = umma::smem_desc(umma::smem_u32(bstride), tc::kBChunk, 128u);
+#pragma unroll 1
+  for (u64 b = lane; b < nblk; b += K) {
+    u32 z[20];
+    tile.collect(z);
+    tc::reduce_z(z, x);
+    if (b + K < nblk) tile.issue(x);
+    to_ranlux_hot(x, v, c);
+    if (live) EmitBlock<0, MODE, OUT>::all(sink, v, b * 12);
+    if (b + 1 == nblk) {  // uniform: this lane ends on the tile's last block
+      if (threadIdx.x == 0) {
+        u32 readers;
+        do {
+          asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(readers) : "l"(a.lane_sync + tidx) : "memory");
+        } while (readers < K);
+        a.lane_sync[tidx] = 0;
+      }
+      __syncthreads();
+      if (live) store_state(a.st, a.n_total, a.first + il, x, 12u);
+    }
+  }
+  tile.teardown();
+}
+
 // Fused sum / sum of squares (S8 a-7b, cfg5) with TWO tiles per CTA on one accumulator (tc::PairTile): nothing is
 // stored, so the kernel is a chain of advances per tile, and interleaving two chains hides the tensor pipe's round
 // trip behind the other tile's integer work.  Work item = (PAIR of adjacent tiles, chunk of draws); n_tiles counts pairs.
@@ -998,12 +1071,16 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_k
 #ifndef RLXPP_PAIR_SYNC
 #define RLXPP_PAIR_SYNC tc::kSyncCta
 #endif
-template <bool ALIGNED>
+template <bool ALIGNED, int MODE = kReduce, int OUT = kF64>
 __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kernel(const __grid_constant__ GenArgs a) {
+  static_assert(MODE == kReduce || MODE == kStoreInterleaved, "pairs: fused reduce or interleaved stores");
   __shared__ tc::PairSmem smem;
   tc::PairTile<RLXPP_PAIR_SYNC> tile;
   tile.setup(smem, a.bmat);
-  const u32 kexp = a.kexp;
+#ifndef RLXPP_STORE_KEXP_PARAM
+#define RLXPP_STORE_KEXP_PARAM 0
+#endif
+  const u32 kexp = (MODE == kReduce || RLXPP_STORE_KEXP_PARAM) ? a.kexp : kExp16;
   const u64 n_items = (u64)a.n_tiles * a.n_chunks;
   for (;;) {
     if (threadIdx.x == 0) smem.ticket = atomicAdd(a.sched, 1u);
@@ -1026,7 +1103,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
     u64 il[2];
     bool live[2], early[2];
     u32 pos[2], newpos[2];
-    Sink<kReduce> sink[2];
+    Sink<MODE, OUT> sink[2];
     u32 x[18], v[18], c;
 #pragma unroll
     for (int t = 0; t < 2; t++) {
@@ -1036,12 +1113,14 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
 #pragma unroll
       for (int j = 0; j < 18; j++) x[j] = 0;
       if (live[t]) load_state(a.st, a.n_total, a.first + il[t], x, pos[t]);
-      sink[t].p = nullptr;
-      sink[t].ld = 0;
+      if (MODE == kStoreInterleaved && OUT == kF32)
+        sink[t].p = reinterpret_cast<double*>(reinterpret_cast<float*>(a.out) + il[t] + 2 * t0 * a.ld);
+      else sink[t].p = MODE == kStoreInterleaved ? a.out + il[t] + t0 * a.ld : nullptr;
+      sink[t].ld = a.ld;
       sink[t].kexp = kexp;
       sink[t].S = 0.0;
       sink[t].Q = 0.0;
-      if (chunk > 0 && live[t]) {
+      if (MODE == kReduce && chunk > 0 && live[t]) {
         sink[t].S = __ldcg(a.sum + il[t]);
         sink[t].Q = __ldcg(a.sumsq + il[t]);
       }
@@ -1050,7 +1129,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
       newpos[t] = (u32)((u64)pos[t] + n - 12 * last);
       if (!ALIGNED && n > 0 && pos[t] < 12) {  // block 0 = the current block
         to_ranlux_exact(x, v, c);
-        if (live[t]) EmitBlock<0, kReduce>::masked(sink[t], v, 0, pos[t], n);
+        if (live[t]) EmitBlock<0, MODE, OUT>::masked(sink[t], v, 0, pos[t], n);
       }
       tile.stash(t, x);
     }
@@ -1069,7 +1148,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
           if (b + 1 < nblk) tile.stash(t, x);
           else if (live[t]) store_state(a.st, a.n_total, a.first + il[t], x, 12u);
           to_ranlux_hot(x, v, c);
-          if (live[t]) EmitBlock<0, kReduce>::all(sink[t], v, 0);
+          if (live[t]) EmitBlock<0, MODE, OUT>::all(sink[t], v, b * 12);
         }
       }
     } else if (n > 0) {
@@ -1087,7 +1166,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
           tc::reduce_z(z, x);
           tile.stash(t, x);
           to_ranlux_hot(x, v, c);
-          if (live[t]) EmitBlock<0, kReduce>::template all<false>(sink[t], v, 0);
+          if (live[t]) EmitBlock<0, MODE, OUT>::template all<false>(sink[t], v, s * 12 - pos[t]);
         }
       }
       // the last two blocks carry per-draw masks; a stream that ends one block early (early[t]) discards the last
@@ -1105,7 +1184,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
           if (!(s == smax && early[t])) {
             if (live[t]) store_state(a.st, a.n_total, a.first + il[t], x, newpos[t]);
             to_ranlux_hot(x, v, c);
-            if (live[t]) EmitBlock<0, kReduce>::masked(sink[t], v, s * 12, pos[t], n);
+            if (live[t]) EmitBlock<0, MODE, OUT>::masked(sink[t], v, s * 12, pos[t], n);
           }
         }
       }
@@ -1118,8 +1197,10 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kern
         q.z = newpos[t];
         a.st[4 * a.n_total + a.first + il[t]] = q;
       }
-      a.sum[il[t]] = sink[t].S;
-      if (a.sumsq) a.sumsq[il[t]] = sink[t].Q;
+      if (MODE == kReduce) {
+        a.sum[il[t]] = sink[t].S;
+        if (a.sumsq) a.sumsq[il[t]] = sink[t].Q;
+      }
     }
     if (a.n_chunks > 1) {  // publish: state and partial sums of this pair are in global memory
       __threadfence();
@@ -1479,6 +1560,40 @@ static int get_bmatrix(uint32_t p, const uint4** out) {
   return RLXPP_OK;
 }
 
+// Images of the byte matrices of A^1 .. A^kMaxLanes (time-parallel path), one set per (device, p), built on first use.
+static std::vector<BmatEntry> g_bmat_pow_cache;
+static int get_bmatrix_powers(uint32_t p, const uint4** out) {
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_bmat_mutex);
+  for (const BmatEntry& e : g_bmat_pow_cache)
+    if (e.dev == dev && e.p == p) { *out = e.ptr; return RLXPP_OK; }
+  std::vector<uint8_t> all((size_t)kMaxLanes * tc::kBBytes, 0);
+  const host::Big A = host::multiplier_ap(p);
+  host::Big R0 = A;  // A^(k + 1)
+  for (u32 k = 0; k < kMaxLanes; k++) {
+    host::Big R = R0;
+    uint8_t* img = all.data() + (size_t)k * tc::kBBytes;
+    for (int col = 0; col < 72; col++) {
+      uint32_t w[18];
+      R.to_u32x18(w);
+      for (int n = 0; n < 72; n++) img[tc::b_offset(n, col)] = (uint8_t)(w[n / 4] >> (8 * (n % 4)));
+      R = host::reduce(host::Big::shl(R, 8));
+    }
+    R0 = host::mulmod(R0, A);
+  }
+  uint4* d = nullptr;
+  CUDA_TRY(cudaMalloc(&d, all.size()));
+  cudaError_t e = cudaMemcpy(d, all.data(), all.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(d);
+    return fail(RLXPP_ECUDA, "uploading the byte matrices of A^k: %s", cudaGetErrorString(e));
+  }
+  g_bmat_pow_cache.push_back({dev, p, d});
+  *out = d;
+  return RLXPP_OK;
+}
+
 // engine used by advance_states / generate_*: the tensor-core path unless told otherwise
 static std::atomic<int> g_engine{RLXPP_ENGINE_UMMA};
 // > 0: cut every tile into this many chunks whatever plan_items says (rlxpp_set_chunks; tests)
@@ -1515,6 +1630,7 @@ struct rlxpp {
   uint32_t* tabG = nullptr;
   const uint4* bmat = nullptr;  // owned by the process-wide cache
   uint32_t* sched = nullptr;    // scheduler words of the persistent UMMA kernel: 1 + ceil(n / 128)
+  uint32_t* lane_sync = nullptr;  // time-parallel path: one reader counter per tile, zero between launches
   double* scratch_q = nullptr;  // sum of squares when the caller passes none (chunked reduce carries it)
   Tables tables;
   bool aligned = true;  // every cursor is known to be 12
@@ -1658,9 +1774,29 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     if (rc) return rc;
   }
   // the fused reduce runs two tiles per CTA (tc_reduce_pair_kernel): its work items are pairs of tiles
-  const uint64_t n_tiles = MODE == kReduce ? (a.count + 2 * tc::kTile - 1) / (2 * tc::kTile) : (a.count + tc::kTile - 1) / tc::kTile;
+#ifndef RLXPP_STORE_PAIRS
+#define RLXPP_STORE_PAIRS 0
+#endif
+  constexpr bool kPairs = MODE == kReduce || (MODE == kStoreInterleaved && OUT == kF64 && RLXPP_STORE_PAIRS);
+  const uint64_t n_tiles = kPairs ? (a.count + 2 * tc::kTile - 1) / (2 * tc::kTile) : (a.count + tc::kTile - 1) / tc::kTile;
   const unsigned slots = tc_slots();
   a.n_tiles = (u32)n_tiles;
+  if constexpr (MODE != kReduce) {
+    // Short calls that leave most of the grid empty: K lanes per tile, each reaching its blocks with the matrices of
+    // A^(j+1) and A^K (tc_generate_lanes_kernel).  All CTAs must be co-resident (the last lane waits for its tile's
+    // readers): n_tiles K <= slots.  rlxpp_set_chunks(c > 0) keeps the persistent path.
+    const uint64_t nblk = a.n_per / 12;
+    uint64_t K = nblk < kMaxLanes ? nblk : kMaxLanes;
+    if (K > slots / n_tiles) K = slots / n_tiles;
+    if (aligned && a.lane_sync && K >= 4 && g_force_chunks.load() == 0) {
+      int rc = get_bmatrix_powers(a.p, &a.bmat_pow);
+      if (rc) return rc;
+      a.lanes = (u32)K;
+      tc_generate_lanes_kernel<MODE, OUT><<<(unsigned)(n_tiles * K), tc::kTile, 0, s>>>(a);
+      LAUNCH_CHECK();
+      return RLXPP_OK;
+    }
+  }
   plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len);
   if (g_force_chunks.load() > 0 && a.n_per / 12 >= (uint64_t)g_force_chunks.load()) {  // test hook
     const uint64_t c = (uint64_t)g_force_chunks.load(), blocks = a.n_per / 12;
@@ -1670,9 +1806,9 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   const uint64_t items = n_tiles * a.n_chunks;
   const unsigned grid = (unsigned)(items < slots ? items : slots);
   CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
-  if (MODE == kReduce) {
-    if (aligned) tc_reduce_pair_kernel<true><<<grid, tc::kTile, 0, s>>>(a);
-    else tc_reduce_pair_kernel<false><<<grid, tc::kTile, 0, s>>>(a);
+  if constexpr (kPairs) {
+    if (aligned) tc_reduce_pair_kernel<true, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
+    else tc_reduce_pair_kernel<false, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
   } else if (aligned) {
     constexpr bool kStaged = MODE == kStoreStreamMajor;  // the kernel's kStaged
     // 20 KB static + 33 KB (stream-major boxes) or 36 KB (float-row boxes): above the 48 KB default, 4 CTAs per SM fit
@@ -1809,6 +1945,9 @@ int rlxpp_create(rlxpp_t** hout, uint64_t n_streams, uint64_t seed, uint32_t p, 
   }
   cudaError_t e = cudaMalloc(&h->st, sizeof(uint4) * 5 * n_streams);
   if (e == cudaSuccess) e = cudaMalloc(&h->sched, sizeof(uint32_t) * (1 + (n_streams + tc::kTile - 1) / tc::kTile));
+  const size_t lane_words = (n_streams + tc::kTile - 1) / tc::kTile;
+  if (e == cudaSuccess) e = cudaMalloc(&h->lane_sync, sizeof(uint32_t) * lane_words);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->lane_sync, 0, sizeof(uint32_t) * lane_words, h->stream);
   if (e == cudaSuccess) e = cudaMalloc(&h->tabA, 64 * 18 * sizeof(uint32_t));
   if (e == cudaSuccess) e = cudaMalloc(&h->tabG, 64 * 18 * sizeof(uint32_t));
   if (e == cudaSuccess)
@@ -1838,6 +1977,7 @@ int rlxpp_destroy(rlxpp_t* h) {
   if (h->stream || h->st) cudaStreamSynchronize(h->stream);
   cudaFree(h->st);
   cudaFree(h->sched);
+  cudaFree(h->lane_sync);
   cudaFree(h->scratch_q);
   cudaFree(h->tabA);
   cudaFree(h->tabG);
@@ -1970,6 +2110,7 @@ int rlxpp_generate_doubles(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, i
   GenArgs a;
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = out_dev; a.ld = h->n;
   a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
+  a.lane_sync = h->lane_sync; a.p = h->p;  // whole-handle call: short ones may run time-parallel
   const bool aligned = h->aligned && n_per_stream % 12 == 0;
   int rc = -1;
   if (layout == RLXPP_STREAM_MAJOR && !aligned)
@@ -2010,6 +2151,7 @@ static int generate_other(rlxpp_t* h, void* out_dev, uint64_t n_draws, int layou
   GenArgs a;
   a.st = h->st; a.n_total = h->n; a.first = 0; a.count = h->n; a.out = (double*)out_dev; a.ld = h->n;
   a.n_per = n_draws; a.sum = nullptr; a.sumsq = nullptr; a.A = h->tables.A; a.bmat = h->bmat; a.sched = h->sched;
+  a.lane_sync = h->lane_sync; a.p = h->p;
   const bool aligned = h->aligned && n_draws % 12 == 0;
   int rc = -1;
   if (layout == RLXPP_STREAM_MAJOR && !aligned)

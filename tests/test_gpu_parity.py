@@ -986,3 +986,47 @@ def test_eight_shard_handles_reproduce_one_generator(rlx, torch, oracle, nthread
         check_state(rlx, torch, h, sub, f"shard starting at stream {first}")
         rlx.rlxpp_destroy(h)
     rlx.rlxpp_destroy(one)
+
+
+# ------------------------------------------------------------------------------------- short calls, time-parallel
+@pytest.mark.parametrize("n, blocks", [(1024, 32), (128 * 20 + 77, 32), (128 * 60, 40), (5, 4), (128 * 140 + 3, 7), (700, 100)])
+def test_short_calls_run_time_parallel(rlx, torch, oracle, nthreads, n, blocks):
+    """UMMA engine, calls that leave most of the grid empty (cfg1's shape): K lanes per tile, lane j reaching block j with
+    the byte matrix of A^(j+1) and striding with the one of A^K (rlxpp.cu tc_generate_lanes_kernel; reading D7: block b is
+    to_ranlux(A^(b+1) X)).  One pass per lane (32 blocks, K = 32), several passes (K = 9 / 29 / 4: 60 or 21 tiles; 100 blocks),
+    a 5-stream handle, a grid that is too full for lanes (141 tiles: the persistent path), ragged tiles; every output form
+    and layout; the state each call leaves is the one the next call starts from; guard bands stay untouched."""
+    per = 12 * blocks
+    calls = [("doubles", "sm"), ("doubles", "il"), ("u48", "sm"), ("floats", "il"), ("normal", "il"), ("doubles", "sm")]
+    ref = oracle.streams(inputs.seeds(n, 3), 2048, per * len(calls), want=("ints", "doubles", "state"), nthreads=nthreads)
+    h = rlx.rlxpp_create(n, 3, 2048)
+    for k, (form, lay) in enumerate(calls):
+        sm = lay == "sm"
+        layout = rlx.RLXPP_STREAM_MAJOR if sm else rlx.RLXPP_INTERLEAVED
+        ints = ref["ints"][:, k * per:(k + 1) * per]
+        words = 2 * per if form == "floats" else per
+        dt = {"doubles": torch.float64, "u48": torch.int64, "floats": torch.float32, "normal": torch.float64}[form]
+        buf = torch.full((n * words + 64,), -1, dtype=dt, device="cuda")
+        if form == "doubles":
+            rlx.rlxpp_generate_doubles(h, buf, per, layout)
+        elif form == "u48":
+            rlx.rlxpp_generate_u48(h, buf, per, layout)
+        elif form == "floats":
+            rlx.rlxpp_generate_floats(h, buf, 2 * per, layout)
+        else:
+            rlx.rlxpp_generate_normal(h, buf, per, layout)
+        torch.cuda.synchronize()
+        raw = buf.cpu().numpy()
+        assert np.all(raw[n * words:] == -1), "wrote behind the output buffer"
+        got = raw[:n * words].reshape(n, words) if sm else raw[:n * words].reshape(words, n).T
+        what = f"time-parallel call {k} ({form}, {lay}), n = {n}, {blocks} blocks"
+        if form == "doubles":
+            assert_bits_equal(got, ref["doubles"][:, k * per:(k + 1) * per], what)
+        elif form == "u48":
+            assert np.array_equal(got.view(np.uint64), ints), what
+        elif form == "floats":
+            assert np.array_equal(np.ascontiguousarray(got).view(np.uint32), _floats_of(ints).view(np.uint32)), what
+        else:
+            assert_within_ulps(got, oracle.normals(ints), NORMAL_ULPS, what)
+    check_state(rlx, torch, h, ref, "after time-parallel calls")
+    rlx.rlxpp_destroy(h)
