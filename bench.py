@@ -30,7 +30,7 @@ IMAD_PER_DOUBLE = 27    # 324 / 12 (one LCG operation per 12 
 # Warp instructions the dominant kernel executes per advance of one warp's 32 streams (ncu smsp__inst_executed.sum /
 # (advances / 32) of the committed --set full captures; profiles/ncu_r02_umma.md).  The issue-slot roofline of the
 # kernels that neither HBM nor the tensor pipe binds: one warp instruction per scheduler and clock.
-WARP_INST_PER_ADVANCE = {"normal": 835, "cfg5": 235, "cfg2": 158}
+WARP_INST_PER_ADVANCE = {"normal": 835, "cfg5": 227, "cfg2": 161}
 TRAFFIC_FILE = "profiles/traffic_r02.json"
 SM_COUNT = 148
 IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles per SMSP, 4 SMSPs
@@ -41,8 +41,8 @@ WORKLOADS = {
     "cfg3": (1 << 20, 1536, 2048, "BASELINE configs[2]: 2^20 streams x 1536 doubles, p=2048, interleaved, 12.9 GB/step"),
     "cfg4": (1 << 18, 6144, 2048, "BASELINE configs[3] at p=2048: 2^18 streams x 6144 doubles, interleaved, 12.9 GB/step"),
     "cfg5": (1 << 18, 49152, 2048, "BASELINE configs[4]: 2^18 streams, random 64-bit skips, 49152 doubles fused to sum/sumsq"),
-    "devapi": (1 << 18, 1200, 2048, "SURVEY 8f-1: device-side draw API (include/rlxpp_device.cuh), 2^18 streams with random "
-                                    "cursors, 1200 draws each summed per stream (rlxpp_generate_ragged_reduce, draw_coop)"),
+    "devapi": (1 << 18, 1200, 2048, "SURVEY 8f-1: device-side draw API (include/rlxpp_tile.cuh TileStream), 2^18 streams with random "
+                                    "cursors, 1200 draws each summed per stream (rlxpp_generate_ragged_reduce, cooperative = 3)"),
     "cfg2": ((1 << 20) + 64, 16, 2048, "BASELINE configs[1]: 2^20+64 raw states x 16 advances in place (AoS)"),
 }
 
@@ -291,8 +291,14 @@ def main():
         units = n_streams * n_per
         alg_bytes = units * 8 + 2 * 80 * n_streams  # doubles written + state read and written back
         lay = rlx.RLXPP_INTERLEAVED if args.layout == "interleaved" else rlx.RLXPP_STREAM_MAJOR
-        kernel = (f"tc_generate_kernel<{args.layout}, aligned>" if umma
-                  else f"generate_kernel<Fixed<{p}>, {args.layout}, aligned>")
+        if not umma:
+            kernel = f"generate_kernel<Fixed<{p}>, {args.layout}, aligned>"
+        elif args.workload == "cfg1":
+            kernel = f"tc_generate_lanes_kernel<{args.layout}>"   # short call: time-parallel lanes
+        elif args.layout == "interleaved" and args.output != "f32":
+            kernel = "tc_pair_kernel<aligned, interleaved>"        # two tiles per CTA on one accumulator
+        else:
+            kernel = f"tc_generate_kernel<{args.layout}, aligned>"
 
         if args.output == "u48":
             out = out.view(torch.int64)
@@ -316,7 +322,7 @@ def main():
         Q = torch.empty(n_streams, dtype=torch.float64, device="cuda")
         units = n_streams * n_per
         alg_bytes = (2 * 80 + 16) * n_streams
-        kernel = "tc_generate_kernel<reduce, unaligned>" if umma else f"generate_kernel<Fixed<{p}>, reduce, unaligned>"
+        kernel = "tc_pair_kernel<unaligned, reduce>" if umma else f"generate_kernel<Fixed<{p}>, reduce, unaligned>"
 
         def step():
             rlx.rlxpp_generate_reduce(h, S, Q, n_per)
@@ -329,17 +335,17 @@ def main():
         cnt = torch.full((n_streams,), n_per, dtype=torch.int32, device="cuda")
         units = n_streams * n_per
         alg_bytes = (2 * 80 + 16 + 4) * n_streams
-        kernel = "ragged_kernel<coop, reduce>"
+        kernel = "ragged_tile_kernel<reduce>"  # rlxpp_dev::TileStream (include/rlxpp_tile.cuh): tensor-core advance per CTA
 
         def step():
-            rlx.rlxpp_generate_ragged_reduce(h, cnt, S, Q, True)
+            rlx.rlxpp_generate_ragged_reduce(h, cnt, S, Q, 3)
     else:  # cfg2: raw advances; "doubles" = 12 per advance for the common unit
         h = None
         states = torch.from_numpy(inputs.cfg2_states(1 << 20).view(np.int64)).cuda()
         reps = n_per
         units = n_streams * reps * 12
         alg_bytes = 144 * n_streams
-        kernel = "tc_advance_states_kernel<AoS>" if umma else f"advance_states_kernel<Fixed<{p}>, AoS>"
+        kernel = "tc_advance_states_pair_kernel<AoS>" if umma else f"advance_states_kernel<Fixed<{p}>, AoS>"
 
         def step():
             rlx.rlxpp_advance_states(states, n_streams, p, reps, rlx.RLXPP_AOS)
@@ -512,14 +518,18 @@ def main():
             torch.cuda.synchronize()
             return units / (c0.elapsed_time(c1) / reps * 1e-3)
         per_thread = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h, cnt, S, Q, False))
+        warp_coop = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h, cnt, S, Q, True))
         h2 = rlx.rlxpp_create(n_streams, first_seed, p)  # fresh handle: every cursor 12 (the paper's aligned case)
         aligned_pt = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h2, cnt, S, Q, False))
         aligned_coop = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h2, cnt, S, Q, True))
+        aligned_tile = timed(lambda: rlx.rlxpp_generate_ragged_reduce(h2, cnt, S, Q, 3))
         rlx.rlxpp_destroy(h2)
-        devapi = {"unit": UNIT, "random_cursors_draw_coop": None, "random_cursors_draw": per_thread,
+        devapi = {"unit": UNIT, "random_cursors_tile": None, "random_cursors_draw_coop": warp_coop,
+                  "random_cursors_draw": per_thread, "aligned_cursors_tile": aligned_tile,
                   "aligned_cursors_draw": aligned_pt, "aligned_cursors_draw_coop": aligned_coop,
-                  "what": "PAPER.md lines 174-176: per-thread skipping made the paper's GPU run 7x slower; draw_coop "
-                          "keeps one advance pass per warp and 12 draws whatever the cursors"}
+                  "what": "PAPER.md lines 174-176: per-thread skipping made the paper's GPU run 7x slower.  draw / draw_coop: "
+                          "rlxpp_dev::Stream, the paper's 324 products per thread (draw_coop: one advance pass per warp and 12 "
+                          "draws whatever the cursors); tile: rlxpp_dev::TileStream, one tensor-core pass per CTA of 128 streams"}
 
     # ---------------------------------------------------------------- end to end (host buffers)
     e2e = None
@@ -598,7 +608,7 @@ def main():
             "other_engine": compare,
         }
         if devapi is not None:
-            devapi["random_cursors_draw_coop"] = value
+            devapi["random_cursors_tile"] = value
             line["device_api"] = devapi
         print(json.dumps(line))
     if dist is not None:

@@ -181,7 +181,8 @@ int rlxpp_host_generate(uint64_t* lcg_inout, uint32_t* pos_inout, uint32_t p, ui
 
 /* ---- Device-side draw API -------------------------------
  * include/rlxpp_device.cuh is a header-only per-thread generator for use inside the caller's own
- * kernels (rlxpp_dev::Stream: load / draw / draw_coop / store).  rlxpp_device_view fills the plain
+ * kernels (rlxpp_dev::Stream: load / draw / draw_coop / store); include/rlxpp_tile.cuh adds
+ * rlxpp_dev::TileStream, the same for CTAs of 128 threads with the advance on the tensor cores.  rlxpp_device_view fills the plain
  * struct such kernels take (device pointers owned by the handle, valid until rlxpp_destroy); after it
  * the library assumes nothing about the cursors.  Kernels using the view must be ordered after the
  * handle's pending work (same CUDA stream, or an event). */
@@ -192,7 +193,8 @@ int rlxpp_device_view(rlxpp_t* h, struct rlxpp_view* out_host);
  * entries beyond a stream's count are left untouched); the _reduce form keeps S = S + d and
  * Q = fma(d, d, Q) per stream in draw order (sumsq_dev may be NULL).  cooperative = 1 uses the
  * warp-cooperative advance (draw_coop), 0 the paper's per-thread advance (draw), 2 alternates the two from
- * draw to draw on the same generator (they mix freely); results are identical.
+ * draw to draw on the same generator (they mix freely), 3 the block-cooperative tensor-core advance of
+ * include/rlxpp_tile.cuh (rlxpp_dev::TileStream: one UMMA pass per CTA of 128 streams); results are identical.
  * State and cursors are updated; the draws are the ones rlxpp_generate_doubles would give. */
 int rlxpp_generate_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out_dev, uint64_t ld, int cooperative);
 int rlxpp_generate_ragged_reduce(rlxpp_t* h, const uint32_t* counts_dev, double* sum_dev, double* sumsq_dev,

@@ -39,6 +39,7 @@ typedef struct rlxpp_view {
   uint4* st;          /* state planes: st[g * n + i], g = 0..4 (limbs 4g..4g+3; plane 4: limbs 16, 17, pos, 0) */
   uint64_t n;         /* streams in the handle */
   const uint32_t* A;  /* the 18 little-endian 32-bit limbs of a^p mod m */
+  const uint4* bmat;  /* shared-memory image of the byte matrix of a^p (rlxpp_tile.cuh: TileStream) */
 } rlxpp_view_t;
 
 namespace rlxpp_dev {

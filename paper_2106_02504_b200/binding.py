@@ -204,7 +204,7 @@ def rlxpp_host_generate(lcg: np.ndarray, pos: int, p: int, skip: int, n: int):
 
 class RlxppView(ctypes.Structure):
     """rlxpp_view_t of include/rlxpp_device.cuh: what a kernel using the device API takes."""
-    _fields_ = [("st", ctypes.c_void_p), ("n", ctypes.c_uint64), ("A", ctypes.c_void_p)]
+    _fields_ = [("st", ctypes.c_void_p), ("n", ctypes.c_uint64), ("A", ctypes.c_void_p), ("bmat", ctypes.c_void_p)]
 
 
 def rlxpp_device_view(h: Handle) -> RlxppView:

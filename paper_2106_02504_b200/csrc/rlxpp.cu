@@ -1064,23 +1064,19 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_lanes_k
   tile.teardown();
 }
 
-// Fused sum / sum of squares (S8 a-7b, cfg5) with TWO tiles per CTA on one accumulator (tc::PairTile): nothing is
-// stored, so the kernel is a chain of advances per tile, and interleaving two chains hides the tensor pipe's round
+// Fused sum / sum of squares (S8 a-7b, cfg5) and interleaved stores (cfg3 / cfg4) with TWO tiles per CTA on one
+// accumulator (tc::PairTile): a tile is a chain of advances, and interleaving two chains hides the tensor pipe's round
 // trip behind the other tile's integer work.  Work item = (PAIR of adjacent tiles, chunk of draws); n_tiles counts pairs.
-// Same contract and the same per-stream arithmetic as tc_generate_kernel<kReduce, ...>.
-#ifndef RLXPP_PAIR_SYNC
-#define RLXPP_PAIR_SYNC tc::kSyncCta
-#endif
+// Same contract and the same per-stream arithmetic as tc_generate_kernel.
+// Hand-off (profiles/ab_r02_pairs.md): the fused reduce is indifferent (CTA barrier 1,228, named barrier 1,223 G doubles/s);
+// the store kernels want the named barrier (cfg3 727 vs 759 burst, 633 vs 655 sustained).
 template <bool ALIGNED, int MODE = kReduce, int OUT = kF64>
-__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_reduce_pair_kernel(const __grid_constant__ GenArgs a) {
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(const __grid_constant__ GenArgs a) {
   static_assert(MODE == kReduce || MODE == kStoreInterleaved, "pairs: fused reduce or interleaved stores");
   __shared__ tc::PairSmem smem;
-  tc::PairTile<RLXPP_PAIR_SYNC> tile;
+  tc::PairTile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
   tile.setup(smem, a.bmat);
-#ifndef RLXPP_STORE_KEXP_PARAM
-#define RLXPP_STORE_KEXP_PARAM 0
-#endif
-  const u32 kexp = (MODE == kReduce || RLXPP_STORE_KEXP_PARAM) ? a.kexp : kExp16;
+  const u32 kexp = a.kexp;  // a launch parameter: the PRMT selectors become immediates (arith.cuh)
   const u64 n_items = (u64)a.n_tiles * a.n_chunks;
   for (;;) {
     if (threadIdx.x == 0) smem.ticket = atomicAdd(a.sched, 1u);
@@ -1432,6 +1428,47 @@ __global__ void __launch_bounds__(kThreads) ragged_kernel(const rlxpp_view_t vie
   }
 }
 
+// The same ragged generation with the block-cooperative tensor-core advance of include/rlxpp_tile.cuh
+// (rlxpp_dev::TileStream, cooperative = 3): a CTA of 128 threads = one tile; when some thread is out of numbers the CTA
+// makes one UMMA pass for every thread that holds no spare block.  Reference use of that public API.
+template <bool REDUCE>
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) ragged_tile_kernel(const rlxpp_view_t view, const u32* __restrict__ counts,
+                                                                               double* __restrict__ out, u64 ld,
+                                                                               double* __restrict__ sum, double* __restrict__ sumsq) {
+  __shared__ rlxpp_dev::TileShared sh;
+  __shared__ u32 max_count;
+  rlxpp_dev::TileStream g;
+  g.begin(sh, view);
+  const u64 i = (u64)blockIdx.x * tc::kTile + threadIdx.x;
+  const bool live = i < view.n;
+  g.load(view, i, live);
+  const u32 cnt = live ? counts[i] : 0u;
+  if (threadIdx.x == 0) max_count = 0;
+  __syncthreads();
+  const u32 wmax = __reduce_max_sync(0xFFFFFFFFu, cnt);
+  if ((threadIdx.x & 31u) == 0) atomicMax(&max_count, wmax);
+  __syncthreads();
+  const u32 maxc = max_count;
+  double S = 0.0, Q = 0.0;
+  double* row = REDUCE ? nullptr : out + i * ld;
+#pragma unroll 4
+  for (u32 t = 0; t < maxc; t++) {
+    const double d = g.draw(t < cnt);
+    if (t < cnt) {
+      if (REDUCE) { S = S + d; Q = __fma_rn(d, d, Q); }
+      else row[t] = d;
+    }
+  }
+  if (live) {
+    g.store(view, i);
+    if (REDUCE) {
+      sum[i] = S;
+      if (sumsq) sumsq[i] = Q;
+    }
+  }
+  g.end();
+}
+
 // ----------------------------------------------------------------------------- roofline probes
 // IMAD peak: 8 independent carry chains of IMAD.WIDE.U32.X per thread, nothing else in the loop.
 __global__ void __launch_bounds__(kThreads) imad_peak_kernel(u64* out, u32 iters, u32 seed) {
@@ -1773,11 +1810,9 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     const int rc = encode_stream_major_map(&a.tmap, a.out, a.count, a.n_per, a.pitch ? a.pitch : a.n_per);
     if (rc) return rc;
   }
-  // the fused reduce runs two tiles per CTA (tc_reduce_pair_kernel): its work items are pairs of tiles
-#ifndef RLXPP_STORE_PAIRS
-#define RLXPP_STORE_PAIRS 0
-#endif
-  constexpr bool kPairs = MODE == kReduce || (MODE == kStoreInterleaved && OUT == kF64 && RLXPP_STORE_PAIRS);
+  // the fused reduce and the interleaved stores run two tiles per CTA (tc_pair_kernel): their work items are pairs of
+  // tiles.  (Interleaved floats keep the one-tile kernel with its row boxes, stream-major its staged TMA path.)
+  constexpr bool kPairs = MODE == kReduce || (MODE == kStoreInterleaved && OUT != kF32);
   const uint64_t n_tiles = kPairs ? (a.count + 2 * tc::kTile - 1) / (2 * tc::kTile) : (a.count + tc::kTile - 1) / tc::kTile;
   const unsigned slots = tc_slots();
   a.n_tiles = (u32)n_tiles;
@@ -1785,14 +1820,14 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     // Short calls that leave most of the grid empty: K lanes per tile, each reaching its blocks with the matrices of
     // A^(j+1) and A^K (tc_generate_lanes_kernel).  All CTAs must be co-resident (the last lane waits for its tile's
     // readers): n_tiles K <= slots.  rlxpp_set_chunks(c > 0) keeps the persistent path.
-    const uint64_t nblk = a.n_per / 12;
+    const uint64_t nblk = a.n_per / 12, tiles1 = (a.count + tc::kTile - 1) / tc::kTile;  // lanes work on single tiles
     uint64_t K = nblk < kMaxLanes ? nblk : kMaxLanes;
-    if (K > slots / n_tiles) K = slots / n_tiles;
+    if (K > slots / tiles1) K = slots / tiles1;
     if (aligned && a.lane_sync && K >= 4 && g_force_chunks.load() == 0) {
       int rc = get_bmatrix_powers(a.p, &a.bmat_pow);
       if (rc) return rc;
       a.lanes = (u32)K;
-      tc_generate_lanes_kernel<MODE, OUT><<<(unsigned)(n_tiles * K), tc::kTile, 0, s>>>(a);
+      tc_generate_lanes_kernel<MODE, OUT><<<(unsigned)(tiles1 * K), tc::kTile, 0, s>>>(a);
       LAUNCH_CHECK();
       return RLXPP_OK;
     }
@@ -1807,8 +1842,10 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   const unsigned grid = (unsigned)(items < slots ? items : slots);
   CUDA_TRY(cudaMemsetAsync(a.sched, 0, sizeof(u32) * (1 + (a.n_chunks > 1 ? n_tiles : 0)), s));
   if constexpr (kPairs) {
-    if (aligned) tc_reduce_pair_kernel<true, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
-    else tc_reduce_pair_kernel<false, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
+    // (Row boxes through the TMA instead of the direct stores were tried for the 8-byte outputs: same burst rate, and
+    // under the power cap NOT better -- doubles 663 vs 662, 48-bit integers 676 vs 704 G/s sustained; profiles/ab_r02_pairs.md.)
+    if (aligned) tc_pair_kernel<true, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
+    else tc_pair_kernel<false, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
   } else if (aligned) {
     constexpr bool kStaged = MODE == kStoreStreamMajor;  // the kernel's kStaged
     // 20 KB static + 33 KB (stream-major boxes) or 36 KB (float-row boxes): above the 48 KB default, 4 CTAs per SM fit
@@ -2355,6 +2392,7 @@ int rlxpp_device_view(rlxpp_t* h, struct rlxpp_view* out_host) {
   out_host->st = h->st;
   out_host->n = h->n;
   out_host->A = h->tabA;  // entry 0 of the power table is A itself
+  out_host->bmat = h->bmat;
   // kernels of the caller may move the cursors: the library no longer knows them
   h->pos_uniform = false;
   h->aligned = false;
@@ -2367,6 +2405,12 @@ static int launch_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out, ui
   int rc = rlxpp_device_view(h, &view);
   if (rc) return rc;
   const unsigned grid = grid_for(h->n);
+  if (coop == 3) {
+    if (reduce) ragged_tile_kernel<true><<<grid, tc::kTile, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    else ragged_tile_kernel<false><<<grid, tc::kTile, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+    LAUNCH_CHECK();
+    return RLXPP_OK;
+  }
   if (reduce) {
     if (coop == 2) ragged_kernel<2, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
     else if (coop) ragged_kernel<1, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);

@@ -1,123 +1,8 @@
-// Thin PTX wrappers for the sm_100a tensor-core path: tcgen05.mma kind::i8 (SASS UTCIMMA),
-// tensor memory allocation and loads (LDTM), mbarrier completion, proxy fences.
-//
-// Everything here is a one-to-one wrapper of one PTX instruction; the kernel that uses them
-// (umma_path.cuh) explains the protocol.
+// The PTX wrappers of the tensor-core path live in the public header include/rlxpp_tile.cuh (namespace
+// rlxpp_dev::umma), shared by the library's kernels and by rlxpp_dev::TileStream.
 #pragma once
-#include <cstdint>
+#include "../../include/rlxpp_tile.cuh"
 
 namespace rlx {
-namespace umma {
-
-typedef uint32_t u32;
-typedef uint64_t u64;
-
-__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
-
-// Shared-memory matrix descriptor, K-major, no swizzle ("interleave"): the operand is a grid of
-// core matrices of 8 rows x 16 bytes stored as 128 contiguous bytes (row r of the core matrix at
-// byte 16 r).  lbo = byte distance between core matrices adjacent along K, sbo = byte distance
-// between core matrices adjacent along M/N.  Bits: [0,14) address >> 4, [16,30) lbo >> 4,
-// [32,46) sbo >> 4, [46,48) descriptor version = 1 (Blackwell), [61,64) swizzle mode = 0.
-__device__ __forceinline__ u64 smem_desc(u32 saddr, u32 lbo_bytes, u32 sbo_bytes) {
-  return (u64)((saddr & 0x3FFFFu) >> 4) | ((u64)(lbo_bytes >> 4) << 16) | ((u64)(sbo_bytes >> 4) << 32) | (1ull << 46);
-}
-
-// Instruction descriptor of kind::i8 with unsigned 8-bit A and B (format 0), 32-bit integer
-// accumulator (c_format 2 at bits [4,6)), both operands K-major, N >> 3 at [17,23), M >> 4 at [24,29).
-__host__ __device__ constexpr u32 idesc_u8u8_s32(int M, int N) {
-  return (2u << 4) | ((u32)(N >> 3) << 17) | ((u32)(M >> 4) << 24);
-}
-
-// One lane of the (converged) warp: true for exactly one of the lanes in the mask.
-__device__ __forceinline__ bool elect_one() {
-  u32 pred;
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "elect.sync _|p, 0xFFFFFFFF;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t"
-      "}"
-      : "=r"(pred));
-  return pred != 0;
-}
-
-// D[tmem] (+)= A[smem] * B[smem]^T, one CTA; issued by ONE thread on behalf of the CTA.
-__device__ __forceinline__ void mma_i8(u32 d_tmem, u64 adesc, u64 bdesc, u32 idesc, u32 accumulate) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t"
-      "}"
-      :
-      : "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-// arrive on the mbarrier once every tcgen05.mma issued so far by this thread has completed
-// (implies tcgen05.fence::before_thread_sync)
-__device__ __forceinline__ void commit(u32 bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-// generic-proxy shared-memory writes -> visible to the async proxy (the tensor core's operand reads)
-__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-__device__ __forceinline__ void mbar_init(u32 bar, u32 count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_wait(u32 bar, u32 parity) {
-  asm volatile(
-      "{\n\t"
-      ".reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t"
-      "}"
-      :
-      : "r"(bar), "r"(parity)
-      : "memory");
-}
-
-// Tensor memory: whole-warp calls.  ncols: power of two >= 32.  The base address is written to smem.
-__device__ __forceinline__ void tmem_alloc(u32 smem_dst, u32 ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
-}
-// after the CTA's last allocation
-__device__ __forceinline__ void tmem_relinquish() {
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(u32 taddr, u32 ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// tcgen05.ld 32x32b: thread t of warp w receives, from TMEM lane 32 (w % 4) + t, N consecutive
-// 32-bit columns starting at the column in taddr (lane in bits [16,32), column in bits [0,16)).
-// All 72 accumulator columns of this thread's TMEM lane, then tcgen05.wait::ld -- ONE asm block, so
-// that no use of the registers can be scheduled before the wait.
-// taddr_lo: columns 0..63, taddr_hi: columns 64..71 (they may sit in different allocations).
-__device__ __forceinline__ void tmem_ld72_wait(u32 taddr_lo, u32 taddr_hi, u32 (&r)[72]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x64.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32, %33, %34, %35, %36, %37, %38, %39, %40, %41, %42, %43, %44, %45, %46, %47, %48, %49, %50, %51, %52, %53, %54, %55, %56, %57, %58, %59, %60, %61, %62, %63}, [%72];\n\t"
-      "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%64, %65, %66, %67, %68, %69, %70, %71}, [%73];\n\t"
-      "tcgen05.wait::ld.sync.aligned;"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), 
-        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), 
-        "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), 
-        "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31]), 
-        "=r"(r[32]), "=r"(r[33]), "=r"(r[34]), "=r"(r[35]), "=r"(r[36]), "=r"(r[37]), "=r"(r[38]), "=r"(r[39]), 
-        "=r"(r[40]), "=r"(r[41]), "=r"(r[42]), "=r"(r[43]), "=r"(r[44]), "=r"(r[45]), "=r"(r[46]), "=r"(r[47]), 
-        "=r"(r[48]), "=r"(r[49]), "=r"(r[50]), "=r"(r[51]), "=r"(r[52]), "=r"(r[53]), "=r"(r[54]), "=r"(r[55]), 
-        "=r"(r[56]), "=r"(r[57]), "=r"(r[58]), "=r"(r[59]), "=r"(r[60]), "=r"(r[61]), "=r"(r[62]), "=r"(r[63]), 
-        "=r"(r[64]), "=r"(r[65]), "=r"(r[66]), "=r"(r[67]), "=r"(r[68]), "=r"(r[69]), "=r"(r[70]), "=r"(r[71])
-      : "r"(taddr_lo), "r"(taddr_hi)
-      : "memory");
-}
-
-}  // namespace umma
+namespace umma = rlxpp_dev::umma;
 }  // namespace rlx

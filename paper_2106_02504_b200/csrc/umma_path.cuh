@@ -33,16 +33,18 @@
 namespace rlx {
 namespace tc {
 
-constexpr int kTile = 128;                    // streams per CTA = UMMA M
-constexpr int kN = 80;                        // UMMA N (72 byte columns, padded to a multiple of 16)
-constexpr int kKChunks = 6;                   // 16-byte K chunks: 96 bytes of K = 3 MMAs of K = 32
-constexpr u32 kAChunk = kTile * 16;           // bytes of one K chunk of the A tile (16 row groups x 128 B)
-constexpr u32 kBChunk = kN * 16;              // same for B (10 row groups x 128 B)
-constexpr u32 kABytes = kKChunks * kAChunk;   // 12,288
-constexpr u32 kBBytes = kKChunks * kBChunk;   // 7,680
-constexpr u32 kTmemCols = 128;                // power of two >= kN
-constexpr int kCtasPerSm = 4;                 // 4 x 128 = the SM's 512 TMEM columns
-constexpr u32 kIdesc = umma::idesc_u8u8_s32(kTile, kN);
+using rlxpp_dev::tile::kTile;
+using rlxpp_dev::tile::kN;
+using rlxpp_dev::tile::kKChunks;
+using rlxpp_dev::tile::kAChunk;
+using rlxpp_dev::tile::kBChunk;
+using rlxpp_dev::tile::kABytes;
+using rlxpp_dev::tile::kBBytes;
+using rlxpp_dev::tile::kTmemCols;
+using rlxpp_dev::tile::kCtasPerSm;
+using rlxpp_dev::tile::kIdesc;
+using rlxpp_dev::tile::b_offset;
+using rlxpp_dev::tile::normalise;
 
 // How the CTA hands the freshly written A tile to the thread that issues the MMAs.
 //   kSyncCta:    __syncthreads, warp 0 issues.  Every warp waits for the slowest one.
@@ -54,12 +56,6 @@ constexpr u32 kIdesc = umma::idesc_u8u8_s32(kTile, kN);
 //                the raw advance, -6 % on the fused reduce, which therefore keeps kSyncCta.
 enum { kSyncCta = 0, kSyncArrive = 2 };
 
-// Shared-memory image of B (what rlxpp_create uploads, see build_bmatrix on the host side):
-// element (n, k) at byte (k / 16) * kBChunk + (n / 8) * 128 + (n % 8) * 16 + (k % 16).
-__host__ __device__ constexpr u32 b_offset(int n, int k) {
-  return (u32)(k / 16) * kBChunk + (u32)(n / 8) * 128u + (u32)(n % 8) * 16u + (u32)(k % 16);
-}
-
 struct Smem {
   __align__(128) uint8_t a[kABytes];
   __align__(128) uint8_t b[kBBytes];
@@ -67,50 +63,6 @@ struct Smem {
   u32 tmem_slot;
   u32 ticket;                  // work item of the persistent scheduler (rlxpp.cu)
 };
-
-// The 72 accumulator columns of one stream -> Z = sum_n acc_n 2^(8n) as 19 limbs (z[18] < 2^15, z[19] = 0).
-__device__ __forceinline__ void normalise(const u32 (&c)[72], u32 (&z)[20]) {
-  // limb k gets columns 4k .. 4k+3 at byte offsets 0, 8, 16, 24.  e_k = c0 + (c1 << 8) and
-  // o_k = c2 + (c3 << 8) are both < 2^23 + 2^31 < 2^32, so  Z = E + (O << 16)  with E, O the
-  // 18-limb numbers of limbs e_k, o_k: 36 shift-adds, 19 byte permutes, one 19-limb carry chain.
-  u32 e[18], o[18], t[19];
-#pragma unroll
-  for (int k = 0; k < 18; k++) {
-    e[k] = c[4 * k] + (c[4 * k + 1] << 8);
-    o[k] = c[4 * k + 2] + (c[4 * k + 3] << 8);
-  }
-  t[0] = o[0] << 16;
-#pragma unroll
-  for (int k = 1; k < 18; k++) t[k] = __byte_perm(o[k - 1], o[k], 0x5432);
-  t[18] = o[17] >> 16;
-  asm("add.cc.u32 %0, %19, %37;\n\t"
-      "addc.cc.u32 %1, %20, %38;\n\t"
-      "addc.cc.u32 %2, %21, %39;\n\t"
-      "addc.cc.u32 %3, %22, %40;\n\t"
-      "addc.cc.u32 %4, %23, %41;\n\t"
-      "addc.cc.u32 %5, %24, %42;\n\t"
-      "addc.cc.u32 %6, %25, %43;\n\t"
-      "addc.cc.u32 %7, %26, %44;\n\t"
-      "addc.cc.u32 %8, %27, %45;\n\t"
-      "addc.cc.u32 %9, %28, %46;\n\t"
-      "addc.cc.u32 %10, %29, %47;\n\t"
-      "addc.cc.u32 %11, %30, %48;\n\t"
-      "addc.cc.u32 %12, %31, %49;\n\t"
-      "addc.cc.u32 %13, %32, %50;\n\t"
-      "addc.cc.u32 %14, %33, %51;\n\t"
-      "addc.cc.u32 %15, %34, %52;\n\t"
-      "addc.cc.u32 %16, %35, %53;\n\t"
-      "addc.cc.u32 %17, %36, %54;\n\t"
-      "addc.u32 %18, %55, 0;"
-      : "=r"(z[0]), "=r"(z[1]), "=r"(z[2]), "=r"(z[3]), "=r"(z[4]), "=r"(z[5]), "=r"(z[6]), "=r"(z[7]), "=r"(z[8]),
-        "=r"(z[9]), "=r"(z[10]), "=r"(z[11]), "=r"(z[12]), "=r"(z[13]), "=r"(z[14]), "=r"(z[15]), "=r"(z[16]),
-        "=r"(z[17]), "=r"(z[18])
-      : "r"(e[0]), "r"(e[1]), "r"(e[2]), "r"(e[3]), "r"(e[4]), "r"(e[5]), "r"(e[6]), "r"(e[7]), "r"(e[8]), "r"(e[9]),
-        "r"(e[10]), "r"(e[11]), "r"(e[12]), "r"(e[13]), "r"(e[14]), "r"(e[15]), "r"(e[16]), "r"(e[17]), "r"(t[0]),
-        "r"(t[1]), "r"(t[2]), "r"(t[3]), "r"(t[4]), "r"(t[5]), "r"(t[6]), "r"(t[7]), "r"(t[8]), "r"(t[9]), "r"(t[10]),
-        "r"(t[11]), "r"(t[12]), "r"(t[13]), "r"(t[14]), "r"(t[15]), "r"(t[16]), "r"(t[17]), "r"(t[18]));
-  z[19] = 0;
-}
 
 template <int SYNC>
 struct Tile {

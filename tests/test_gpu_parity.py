@@ -461,14 +461,16 @@ def test_p24_floats_are_the_raw_ranlux_numbers(rlx, torch, oracle):
 
 
 # ------------------------------------------------------------------------------------- device API (8f-1)
-@pytest.mark.parametrize("coop", [True, False, 2])
+@pytest.mark.parametrize("coop", [True, False, 2, 3])
 def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, coop):
     """include/rlxpp_device.cuh through rlxpp_generate_ragged: every stream draws its own number of
     doubles (0 .. 70, so lanes of a warp run out of their blocks at different calls), from per-stream
     cursors, twice in a row, then the library's bulk kernel continues the same streams.  Everything
     must be the one sequence the oracle gives for that stream; cooperative and per-thread advance agree,
     and so does a kernel that alternates draw_coop() and draw() on the same Stream (coop = 2: a spare block
-    made by draw_coop() must be entered, not recomputed past, by draw())."""
+    made by draw_coop() must be entered, not recomputed past, by draw()); coop = 3 is include/rlxpp_tile.cuh's
+    rlxpp_dev::TileStream, the block-cooperative tensor-core advance (ragged counts: threads ask for passes at different
+    calls, some threads of a CTA are done long before others, the last CTA is ragged)."""
     n, p, ld = 1000, 2048, 72
     dist = inputs.splitmix64(77, n) % np.uint64(30)
     c1 = (inputs.splitmix64(78, n) % np.uint64(71)).astype(np.uint32)
@@ -495,7 +497,7 @@ def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, 
     rlx.rlxpp_destroy(h)
 
 
-@pytest.mark.parametrize("coop", [True, False, 2])
+@pytest.mark.parametrize("coop", [True, False, 2, 3])
 def test_device_api_ragged_reduce(rlx, torch, oracle, nthreads, coop):
     n, p = 700, 389
     cnt = (inputs.splitmix64(5150, n) % np.uint64(200)).astype(np.uint32)

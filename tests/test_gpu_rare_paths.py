@@ -130,6 +130,24 @@ def model_counts(engine, oracle, x0s, n_fold, n_hot, pad_to=128):
     return cnt
 
 
+def model_counts_lanes(oracle, x0s, nblk):
+    """UMMA engine, time-parallel path with one lane per block (tc_generate_lanes_kernel, K = nblk): block j of a stream is
+    ONE pass from the stored state against the byte matrix of A^(j+1), so the product that is folded is
+    sum_k xb_k (A^(j+1) 2^(8k) mod m), not a chain of products by A."""
+    cnt = np.zeros(8, np.uint64)
+    cnt[NEAR] += ((-len(x0s)) % 128) * nblk
+    for j in range(1, nblk + 1):
+        Aj = pow(A, j, M)
+        rows = [(Aj << (8 * k)) % M for k in range(72)]
+        for x0 in x0s:
+            fm = fold_mask(sum(((x0 >> (8 * k)) & 0xFF) * rows[k] for k in range(72)))
+            rm = ranlux_mask(Aj * x0 % M, oracle)
+            mask = fm | (rm if rm & FAST_BITS else 0)
+            for k in range(8):
+                cnt[k] += (mask >> k) & 1
+    return cnt
+
+
 # ------------------------------------------------------------------------------------- crafted target states
 def crafted_targets():
     """(family, X_t) pairs; X_t canonical (< m)."""
@@ -275,15 +293,17 @@ def test_crafted_states_hit_what_they_are_crafted_for(oracle):
 
 
 @gpu
-@pytest.mark.parametrize("mode", ["stream_major_short", "stream_major_tma", "interleaved", "reduce", "floats_boxes", "u48",
-                                  "chunked"])
+@pytest.mark.parametrize("mode", ["stream_major_short", "stream_major_tma", "interleaved", "interleaved_odd", "reduce",
+                                  "floats_boxes", "u48", "chunked", "lanes"])
 def test_rare_branches_aligned(rlx, torch, oracle, engine, mode):
-    """Aligned cursors (pos = 12, whole blocks): the pipelined loop of tc_generate_kernel<.., aligned> / generate_kernel
-    <.., aligned>.  The crafted state is produced by advance d in {1, 2, 3, nblk}."""
-    nblk = {"stream_major_short": 4, "stream_major_tma": 17, "interleaved": 4, "reduce": 5, "floats_boxes": 4, "u48": 4,
-            "chunked": 32}[mode]
-    n = 4 * 128 + 44 if mode != "chunked" else 3 * 128 + 44
-    depths = (1, 2, 3, nblk) if mode != "chunked" else (1, 16, 17, 32)
+    """Aligned cursors (pos = 12, whole blocks): the pipelined loops of tc_generate_kernel<.., aligned> (stream-major,
+    floats), tc_pair_kernel<aligned, ..> (interleaved, even and odd stream counts; fused reduce) and generate_kernel<.., aligned> (IMAD), kept on the serial path with rlxpp_set_chunks; the crafted state is
+    produced by advance d in {1, 2, 3, nblk}.  `lanes`: the time-parallel path such short calls take by default, where
+    block d is one pass against the matrix of A^d."""
+    nblk = {"stream_major_short": 4, "stream_major_tma": 17, "interleaved": 4, "interleaved_odd": 4, "reduce": 5,
+            "floats_boxes": 4, "u48": 4, "chunked": 32, "lanes": 32}[mode]
+    n = {"chunked": 3 * 128 + 44, "lanes": 3 * 128 + 44, "interleaved_odd": 4 * 128 + 45}.get(mode, 4 * 128 + 44)
+    depths = {"chunked": (1, 16, 17, 32), "lanes": (1, 2, 17, 32)}.get(mode, (1, 2, 3, nblk))
     x0s, info = build_streams(n, depths)
     per = 12 * nblk
     h = rlx.rlxpp_create(n, 1, P)
@@ -291,14 +311,14 @@ def test_rare_branches_aligned(rlx, torch, oracle, engine, mode):
     ints, xe, pe = oracle_run(oracle, x0s, [12] * n, per)
     want = ints.astype(np.float64) * 2.0**-48
     rlx.rlxpp_rare_counts(reset=True)
-    if mode == "chunked":
-        rlx.rlxpp_set_chunks(2)
+    if mode != "lanes":  # a forced chunk count keeps the call on the persistent kernels
+        rlx.rlxpp_set_chunks(2 if mode == "chunked" else 1)
     try:
-        if mode in ("stream_major_short", "stream_major_tma", "chunked"):
+        if mode in ("stream_major_short", "stream_major_tma", "chunked", "lanes"):
             out = torch.empty((n, per), dtype=torch.float64, device="cuda")
             rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_STREAM_MAJOR)
             assert np.array_equal(out.cpu().numpy().view(np.uint64), want.view(np.uint64)), mode
-        elif mode == "interleaved":
+        elif mode in ("interleaved", "interleaved_odd"):
             out = torch.empty((per, n), dtype=torch.float64, device="cuda")
             rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
             assert np.array_equal(out.cpu().numpy().T.copy().view(np.uint64), want.view(np.uint64)), mode
@@ -324,8 +344,12 @@ def test_rare_branches_aligned(rlx, torch, oracle, engine, mode):
         rlx.rlxpp_set_chunks(0)
     # u48 and floats always run the UMMA engine's kernels (include/rlxpp.h)
     eng = "umma" if mode in ("u48", "floats_boxes") else engine
-    pad_to = 256 if mode == "reduce" else 128  # the fused reduce runs two tiles per CTA (tc_reduce_pair_kernel)
-    assert_counts(rlx, model_counts(eng, oracle, x0s, [nblk] * n, [nblk] * n, pad_to), f"aligned {mode}", ALL_HOT)
+    pad_to = 256 if mode in ("reduce", "interleaved", "interleaved_odd") else 128  # two tiles per CTA (tc_pair_kernel)
+    if mode == "lanes" and eng == "umma":
+        want_counts = model_counts_lanes(oracle, x0s, nblk)
+    else:
+        want_counts = model_counts(eng, oracle, x0s, [nblk] * n, [nblk] * n, pad_to)
+    assert_counts(rlx, want_counts, f"aligned {mode}", ALL_HOT)
     check_final_state(rlx, torch, oracle, h, xe, pe, f"aligned {mode}")
     rlx.rlxpp_destroy(h)
 
@@ -385,7 +409,7 @@ def test_rare_branches_unaligned(rlx, torch, oracle, engine, mode, cursors):
     # IMAD: a thread advances only up to its own last block
     n_fold = [smax] * n if engine == "umma" else last
     needed = ALL_HOT if cursors == "five" else ()
-    pad_to = 256 if mode == "reduce" else 128
+    pad_to = 256 if mode in ("reduce", "interleaved") else 128
     assert_counts(rlx, model_counts(engine, oracle, x0s, n_fold, last, pad_to), f"unaligned {mode} {cursors}", needed)
     check_final_state(rlx, torch, oracle, h, xe, pe, f"unaligned {mode}")
     rlx.rlxpp_destroy(h)
@@ -431,4 +455,36 @@ def test_counters_stay_zero_on_ordinary_streams_and_reset(rlx, torch):
     c = rlx.rlxpp_rare_counts(reset=True)
     assert sum(c.tolist()) == int(c[RCARRY]) <= 3
     assert rlx.rlxpp_rare_counts().tolist() == [0] * 8
+    rlx.rlxpp_destroy(h)
+
+
+@gpu
+@pytest.mark.parametrize("coop", [1, 3])
+def test_rare_branches_device_api(rlx, torch, oracle, engine, coop):
+    """The public device headers on the crafted states: rlxpp_dev::TileStream (include/rlxpp_tile.cuh, coop = 3) runs the
+    same fast forms with the same exact fallbacks inside its tensor-core pass (no counters there: parity only);
+    rlxpp_dev::Stream (coop = 1) is exact arithmetic throughout.  Every stream draws its own count from its own cursor."""
+    if engine != "umma":
+        pytest.skip("the device API does not depend on the library's engine switch")
+    n = 3 * 128 + 77
+    x0s, info = build_streams(n, (1, 2, 3, 4))
+    pos = (inputs.splitmix64(1234, n) % np.uint64(13)).astype(np.int32)
+    pos[::3] = 12
+    cnt = (40 + inputs.splitmix64(99, n) % np.uint64(20)).astype(np.uint32)  # 40 .. 59 draws: 4 or 5 passes
+    ld = 64
+    h = rlx.rlxpp_create(n, 1, P)
+    rlx.rlxpp_set_state(h, to_dev(torch, x0s), torch.from_numpy(pos).cuda())
+    out = torch.full((n, ld), -1.0, dtype=torch.float64, device="cuda")
+    rlx.rlxpp_generate_ragged(h, torch.from_numpy(cnt.view(np.int32)).cuda(), out, ld, coop)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    xe, pe = [], []
+    for i in range(n):
+        X, p_, d = oracle.engine_run(x0s[i], int(pos[i]), P, [("draw", int(cnt[i]))])
+        want = np.array(d, np.uint64).astype(np.float64) * 2.0**-48
+        assert np.array_equal(got[i, :cnt[i]].view(np.uint64), want.view(np.uint64)), f"stream {i} ({info[i][0]})"
+        assert np.all(got[i, cnt[i]:] == -1.0)
+        xe.append(X)
+        pe.append(p_)
+    check_final_state(rlx, torch, oracle, h, xe, pe, f"device API coop = {coop}")
     rlx.rlxpp_destroy(h)

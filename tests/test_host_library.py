@@ -123,15 +123,17 @@ def test_host_engine_matches_big_integer_model(p):
         rlx.rlxpp_host_generate(_limbs(1), 13, p, 0, 1)
 
 
-def test_public_device_header_is_self_contained(tmp_path):
-    """include/rlxpp_device.cuh alone is enough to write a kernel: nvcc compiles a user
-    kernel that includes nothing else (cross-compilation for sm_100a, no GPU needed)."""
+@pytest.mark.parametrize("example", ["device_api_example.cu", "tile_api_example.cu"])
+def test_public_device_header_is_self_contained(tmp_path, example):
+    """include/rlxpp_device.cuh (per-thread generator) and include/rlxpp_tile.cuh (block-cooperative tensor-core
+    advance) alone are enough to write a kernel: nvcc compiles a user kernel that includes nothing else
+    (cross-compilation for sm_100a, no GPU needed)."""
     import shutil
     import subprocess
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
     if not os.path.exists(nvcc):
         pytest.skip("nvcc not found")
-    src = os.path.join(ROOT, "tests", "data", "device_api_example.cu")
+    src = os.path.join(ROOT, "tests", "data", example)
     res = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-I", os.path.join(ROOT, "include"),
                           "-c", src, "-o", str(tmp_path / "example.o")], capture_output=True, text=True)
     assert res.returncode == 0, res.stdout + res.stderr
