@@ -345,7 +345,7 @@ def main():
         reps = n_per
         units = n_streams * reps * 12
         alg_bytes = 144 * n_streams
-        kernel = "tc_advance_states_pair_kernel<AoS>" if umma else f"advance_states_kernel<Fixed<{p}>, AoS>"
+        kernel = "tc_advance_states_group_kernel<AoS>" if umma else f"advance_states_kernel<Fixed<{p}>, AoS>"
 
         def step():
             rlx.rlxpp_advance_states(states, n_streams, p, reps, rlx.RLXPP_AOS)

@@ -171,27 +171,32 @@ struct Generic {
 // coalesced accesses to/from shared memory, each thread picks up its 72 bytes there (stride 18
 // words: 2-way bank conflict).  SoA: limb-major planes, coalesced directly.
 constexpr int kRawStageWords = kThreads * 72 / 16;
-template <int LAYOUT>
-__device__ __forceinline__ void load_raw(const u64* __restrict__ states, u64 n, uint4* stage, u32 (&x)[18], u64 blk) {
+// tid = thread within the 128 that own the tile, sync() = barrier over them (a CTA, or one group of a larger CTA)
+struct CtaSync {
+  __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+template <int LAYOUT, class SYNC = CtaSync>
+__device__ __forceinline__ void load_raw(const u64* __restrict__ states, u64 n, uint4* stage, u32 (&x)[18], u64 blk,
+                                         u32 tid = threadIdx.x, SYNC sync = SYNC()) {
   const u64 base = blk * kThreads;
-  const u64 i = base + threadIdx.x;
+  const u64 i = base + tid;
 #pragma unroll
   for (int j = 0; j < 18; j++) x[j] = 0;
   if (LAYOUT == RLXPP_AOS) {
     const u64 cnt = (n - base < (u64)kThreads ? n - base : (u64)kThreads) * 72 / 8;  // u64 words
     const uint4* src = reinterpret_cast<const uint4*>(states + base * 9);
-    for (u32 q = threadIdx.x; q < (cnt + 1) / 2; q += kThreads) {
+    for (u32 q = tid; q < (cnt + 1) / 2; q += kThreads) {
       if (2 * (u64)q + 1 < cnt) stage[q] = src[q];
       else {  // odd tail: last 8 bytes
         const u64 lastw = states[base * 9 + 2 * (u64)q];
         stage[q] = make_uint4((u32)lastw, (u32)(lastw >> 32), 0u, 0u);
       }
     }
-    __syncthreads();
+    sync();
     const u32* sw = reinterpret_cast<const u32*>(stage);
     if (i < n) {
 #pragma unroll
-      for (int j = 0; j < 18; j++) x[j] = sw[threadIdx.x * 18 + j];
+      for (int j = 0; j < 18; j++) x[j] = sw[tid * 18 + j];
     }
   } else if (i < n) {
 #pragma unroll
@@ -202,21 +207,22 @@ __device__ __forceinline__ void load_raw(const u64* __restrict__ states, u64 n, 
     }
   }
 }
-template <int LAYOUT>
-__device__ __forceinline__ void store_raw(u64* __restrict__ states, u64 n, uint4* stage, const u32 (&x)[18], u64 blk) {
+template <int LAYOUT, class SYNC = CtaSync>
+__device__ __forceinline__ void store_raw(u64* __restrict__ states, u64 n, uint4* stage, const u32 (&x)[18], u64 blk,
+                                          u32 tid = threadIdx.x, SYNC sync = SYNC()) {
   const u64 base = blk * kThreads;
-  const u64 i = base + threadIdx.x;
+  const u64 i = base + tid;
   if (LAYOUT == RLXPP_AOS) {
-    __syncthreads();
+    sync();
     u32* sw = reinterpret_cast<u32*>(stage);
     if (i < n) {
 #pragma unroll
-      for (int j = 0; j < 18; j++) sw[threadIdx.x * 18 + j] = x[j];
+      for (int j = 0; j < 18; j++) sw[tid * 18 + j] = x[j];
     }
-    __syncthreads();
+    sync();
     const u64 cnt = (n - base < (u64)kThreads ? n - base : (u64)kThreads) * 72 / 8;
     uint4* dst = reinterpret_cast<uint4*>(states + base * 9);
-    for (u32 q = threadIdx.x; q < (cnt + 1) / 2; q += kThreads) {
+    for (u32 q = tid; q < (cnt + 1) / 2; q += kThreads) {
       if (2 * (u64)q + 1 < cnt) dst[q] = stage[q];
       else states[base * 9 + 2 * (u64)q] = (u64)stage[q].x | ((u64)stage[q].y << 32);
     }
@@ -968,35 +974,6 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
   tile.teardown();
 }
 
-template <int LAYOUT>
-__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_kernel(u64* __restrict__ states, u64 n, u32 reps,
-                                                                        const uint4* __restrict__ bmat) {
-  static_assert(tc::kTile == kThreads, "raw state I/O assumes 128 threads");
-  __shared__ tc::Smem smem;
-  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kRawStageWords : 1];
-  tc::Tile<tc::kSyncArrive> tile;
-  tile.setup(smem, bmat);
-  const u64 n_tiles = (n + kThreads - 1) / kThreads;
-  // persistent: TMEM allocation and the B matrix are set up once per CTA, tiles are strided over the grid
-#pragma unroll 1
-  for (u64 blk = blockIdx.x; blk < n_tiles; blk += gridDim.x) {
-    u32 x[18];
-    load_raw<LAYOUT>(states, n, stage, x, blk);
-    if (reps == 0) canonicalise(x);
-    else tile.issue(x);
-#pragma unroll 1
-    for (u32 r = 0; r < reps; r++) {
-      u32 z[20];
-      tile.collect(z);
-      tc::reduce_z(z, x);
-      if (r + 1 < reps) tile.issue(x);
-    }
-    store_raw<LAYOUT>(states, n, stage, x, blk);
-    __syncthreads();  // the staging buffer is reused by the next tile
-  }
-  tile.teardown();
-}
-
 // Short calls (cfg1: 8 tiles x 32 blocks, S8d "launch-latency dominated"): a tile's blocks are a serial chain only if
 // they are computed one from the other.  Block b of a stream is to_ranlux(A^(b+1) X) (D7; "fast exponentiation"),
 // so with the byte matrices of A^1 .. A^K at hand, K CTAs ("lanes") work on ONE tile at once: lane j reads the stored
@@ -1070,28 +1047,29 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_lanes_k
 // Same contract and the same per-stream arithmetic as tc_generate_kernel.
 // Hand-off (profiles/ab_r02_pairs.md): the fused reduce is indifferent (CTA barrier 1,228, named barrier 1,223 G doubles/s);
 // the store kernels want the named barrier (cfg3 727 vs 759 burst, 633 vs 655 sustained).
-template <bool ALIGNED, int MODE = kReduce, int OUT = kF64>
-__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(const __grid_constant__ GenArgs a) {
+// The work loop of the 128 threads that own pairs of tiles, written against the tile policy TILE (tc::PairTile): tile.tid =
+// thread within the 128, tile.sync() = barrier over them, tile.ticket = their shared scheduler word, tile.collect() = one
+// half-step.  (The same loop on tc::GroupTile -- 5 groups of 128 threads in one CTA per SM, 80 registers -- was measured
+// for the fused reduce: 1,128 vs 1,230 G doubles/s.  More warps do not help: the ALU pipe binds; profiles/ab_r02_pairs.md.)
+template <bool ALIGNED, int MODE, int OUT, class TILE>
+__device__ __forceinline__ void pair_items(TILE& tile, const GenArgs& a) {
   static_assert(MODE == kReduce || MODE == kStoreInterleaved, "pairs: fused reduce or interleaved stores");
-  __shared__ tc::PairSmem smem;
-  tc::PairTile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
-  tile.setup(smem, a.bmat);
   const u32 kexp = a.kexp;  // a launch parameter: the PRMT selectors become immediates (arith.cuh)
   const u64 n_items = (u64)a.n_tiles * a.n_chunks;
   for (;;) {
-    if (threadIdx.x == 0) smem.ticket = atomicAdd(a.sched, 1u);
-    __syncthreads();
-    const u64 w = smem.ticket;
+    if (tile.tid == 0) *tile.ticket = atomicAdd(a.sched, 1u);
+    tile.sync();
+    const u64 w = *reinterpret_cast<volatile u32*>(tile.ticket);
     if (w >= n_items) break;
     const u32 pidx = (u32)(w % a.n_tiles), chunk = (u32)(w / a.n_tiles);
     if (chunk > 0) {
-      if (threadIdx.x == 0) {
+      if (tile.tid == 0) {
         u32 done;
         do {
           asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(a.sched + 1 + pidx) : "memory");
         } while (done < chunk);
       }
-      __syncthreads();
+      tile.sync();
     }
     const u64 t0 = (u64)chunk * a.chunk_len;
     const u64 n = a.n_per - t0 < a.chunk_len ? a.n_per - t0 : a.chunk_len;
@@ -1103,7 +1081,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(cons
     u32 x[18], v[18], c;
 #pragma unroll
     for (int t = 0; t < 2; t++) {
-      il[t] = ((u64)pidx * 2 + t) * tc::kTile + threadIdx.x;
+      il[t] = ((u64)pidx * 2 + t) * tc::kTile + tile.tid;
       live[t] = il[t] < a.count;
       pos[t] = 12;
 #pragma unroll
@@ -1136,10 +1114,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(cons
       for (u64 b = 0; b < nblk; b++) {
 #pragma unroll
         for (int t = 0; t < 2; t++) {
-          u32 cols[72], z[20];
-          tile.load(cols);
-          if (t == 0 || b + 1 < nblk) tile.start(t ^ 1);  // the other tile's MMA runs under this tile's integer work
-          tc::normalise(cols, z);
+          u32 z[20];
+          tile.collect(z, t == 0 || b + 1 < nblk, t ^ 1);  // the other tile's MMA runs under this tile's integer work
           tc::reduce_z(z, x);
           if (b + 1 < nblk) tile.stash(t, x);
           else if (live[t]) store_state(a.st, a.n_total, a.first + il[t], x, 12u);
@@ -1155,10 +1131,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(cons
       for (; s + 2 <= smax; s++) {
 #pragma unroll
         for (int t = 0; t < 2; t++) {
-          u32 cols[72], z[20];
-          tile.load(cols);
-          tile.start(t ^ 1);
-          tc::normalise(cols, z);
+          u32 z[20];
+          tile.collect(z, true, t ^ 1);
           tc::reduce_z(z, x);
           tile.stash(t, x);
           to_ranlux_hot(x, v, c);
@@ -1171,10 +1145,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(cons
       for (; s <= smax; s++) {
 #pragma unroll
         for (int t = 0; t < 2; t++) {
-          u32 cols[72], z[20];
-          tile.load(cols);
-          if (t == 0 || s < smax) tile.start(t ^ 1);
-          tc::normalise(cols, z);
+          u32 z[20];
+          tile.collect(z, t == 0 || s < smax, t ^ 1);
           tc::reduce_z(z, x);
           if (s < smax) tile.stash(t, x);
           if (!(s == smax && early[t])) {
@@ -1200,40 +1172,59 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(cons
     }
     if (a.n_chunks > 1) {  // publish: state and partial sums of this pair are in global memory
       __threadfence();
-      __syncthreads();
-      if (threadIdx.x == 0)
+      tile.sync();
+      if (tile.tid == 0)
         asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.sched + 1 + pidx), "r"(chunk + 1u) : "memory");
     } else {
-      __syncthreads();  // smem.ticket is rewritten at the top of the loop
+      tile.sync();  // the ticket word is rewritten at the top of the loop
     }
   }
-  tile.teardown();
 }
 
-// Raw advance (cfg2) with two tiles per CTA on one accumulator; one CTA per pair of tiles.
-template <int LAYOUT>
-__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_pair_kernel(u64* __restrict__ states, u64 n, u32 reps,
-                                                                                         const uint4* __restrict__ bmat) {
+template <bool ALIGNED, int MODE = kReduce, int OUT = kF64>
+__global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(const __grid_constant__ GenArgs a) {
   __shared__ tc::PairSmem smem;
-  __shared__ uint4 stage[LAYOUT == RLXPP_AOS ? kRawStageWords : 1];
-  tc::PairTile<tc::kSyncArrive> tile;
+  tc::PairTile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
+  tile.setup(smem, a.bmat);
+  pair_items<ALIGNED, MODE, OUT>(tile, a);
+  tile.teardown();
+}
+// Raw advance (cfg2; S8 a-3 / a-4 alone): x <- A^reps x on raw uint64[9] states, in place.  Two tiles per accumulator
+// (the other tile's MMA runs under this tile's normalisation, as in tc_pair_kernel) and tc::kGroups groups of 128
+// threads in one CTA per SM (tc::GroupTile): six accumulators per SM instead of four.  Persistent: group (CTA c, group g)
+// strides over the pairs of tiles.  Measured at cfg2 (G doubles-equivalent/s): one tile per CTA 1,160; pairs in four
+// CTAs 1,180; 5 groups 1,228; 6 groups 1,320.
+struct GroupSync {
+  u32 barid;
+  __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 128;" ::"r"(barid) : "memory"); }
+};
+template <int LAYOUT>
+__global__ void __launch_bounds__(tc::kGroups * tc::kTile, 1) tc_advance_states_group_kernel(u64* __restrict__ states, u64 n, u32 reps,
+                                                                                          const uint4* __restrict__ bmat) {
+  extern __shared__ __align__(128) uint8_t group_smem[];
+  tc::GroupsSmem& smem = *reinterpret_cast<tc::GroupsSmem*>(group_smem);
+  uint4* stage_all = reinterpret_cast<uint4*>(group_smem + ((sizeof(tc::GroupsSmem) + 127) & ~(size_t)127));
+  tc::GroupTile tile;
   tile.setup(smem, bmat);
+  const u32 gid = threadIdx.x / tc::kTile;
+  uint4* stage = stage_all + (size_t)gid * kRawStageWords;
+  const GroupSync gsync{tile.barid};
   const u64 n_tiles = (n + kThreads - 1) / kThreads, n_pairs = (n_tiles + 1) / 2;
 #pragma unroll 1
-  for (u64 pair = blockIdx.x; pair < n_pairs; pair += gridDim.x) {
+  for (u64 pair = (u64)blockIdx.x * tc::kGroups + gid; pair < n_pairs; pair += (u64)gridDim.x * tc::kGroups) {
     u32 x[18];
 #pragma unroll
     for (int t = 0; t < 2; t++) {
       const u64 blk = 2 * pair + t;
 #pragma unroll
       for (int j = 0; j < 18; j++) x[j] = 0;
-      if (blk < n_tiles) {  // uniform
-        load_raw<LAYOUT>(states, n, stage, x, blk);
+      if (blk < n_tiles) {  // uniform over the group
+        load_raw<LAYOUT>(states, n, stage, x, blk, tile.tid, gsync);
         if (reps == 0) {
           canonicalise(x);
-          store_raw<LAYOUT>(states, n, stage, x, blk);
+          store_raw<LAYOUT>(states, n, stage, x, blk, tile.tid, gsync);
         }
-        __syncthreads();  // the staging buffer is reused
+        gsync();  // the staging buffer is reused
       }
       tile.stash(t, x);
     }
@@ -1242,15 +1233,13 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_advance_states_p
     for (u32 r = 0; r < reps; r++) {
 #pragma unroll
       for (int t = 0; t < 2; t++) {
-        u32 cols[72], z[20];
-        tile.load(cols);
-        if (t == 0 || r + 1 < reps) tile.start(t ^ 1);
-        tc::normalise(cols, z);
+        u32 z[20];
+        tile.collect(z, t == 0 || r + 1 < reps, t ^ 1);
         tc::reduce_z(z, x);
         if (r + 1 < reps) tile.stash(t, x);
         else if (2 * pair + t < n_tiles) {
-          store_raw<LAYOUT>(states, n, stage, x, 2 * pair + t);
-          __syncthreads();
+          store_raw<LAYOUT>(states, n, stage, x, 2 * pair + t, tile.tid, gsync);
+          gsync();
         }
       }
     }
@@ -2072,12 +2061,23 @@ int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, ui
     // one CTA per tile: measured faster than a persistent grid here (1,050 vs 946 G doubles-equivalent/s at
     // cfg2: with 16 advances per tile the load / compute / store phases of co-resident CTAs overlap better when
     // the CTAs are not in lock step); the kernel's tile loop serves grids smaller than the tile count
-    const uint64_t pairs = (tiles + 1) / 2;  // two tiles per CTA on one accumulator (tc::PairTile)
-    const unsigned grid = (unsigned)(pairs < (1u << 30) ? pairs : (1u << 30));
-    if (layout == RLXPP_AOS) tc_advance_states_pair_kernel<RLXPP_AOS><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
-    else tc_advance_states_pair_kernel<RLXPP_SOA><<<grid, tc::kTile, 0, s>>>(states_dev, n_states, reps, bmat);
-    LAUNCH_CHECK();
-    return RLXPP_OK;
+    {  // one CTA per SM with tc::kGroups groups (cfg2: 1,180 with pairs in four CTAs, 1,228 with 5 groups, 1,320 with 6)
+      const size_t smem_bytes = ((sizeof(tc::GroupsSmem) + 127) & ~(size_t)127) +
+                                (layout == RLXPP_AOS ? (size_t)tc::kGroups * kRawStageWords * sizeof(uint4) : 0);
+      const unsigned ctas = tc_slots() / tc::kCtasPerSm;
+      static std::atomic<uint64_t> done_aos{0}, done_soa{0};
+      if (layout == RLXPP_AOS) {
+        rc = allow_dynamic_smem(tc_advance_states_group_kernel<RLXPP_AOS>, done_aos, (int)smem_bytes);
+        if (rc) return rc;
+        tc_advance_states_group_kernel<RLXPP_AOS><<<ctas, tc::kGroups * tc::kTile, smem_bytes, s>>>(states_dev, n_states, reps, bmat);
+      } else {
+        rc = allow_dynamic_smem(tc_advance_states_group_kernel<RLXPP_SOA>, done_soa, (int)smem_bytes);
+        if (rc) return rc;
+        tc_advance_states_group_kernel<RLXPP_SOA><<<ctas, tc::kGroups * tc::kTile, smem_bytes, s>>>(states_dev, n_states, reps, bmat);
+      }
+      LAUNCH_CHECK();
+      return RLXPP_OK;
+    }
   }
 #define RLXPP_CASE(P) \
   if (fixed == P) return launch_advance_mult<Fixed<P>>(states_dev, n_states, reps, layout, t.A, s);

@@ -196,9 +196,14 @@ struct PairTile {
   u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of A tile 0 (tile 1: + kABytes)
   u32 bar, phase, tmem, tld, issuer;
   u64 adesc, bdesc;  // adesc: A tile 0
+  u32 tid;           // thread within the tile (= stream within each of the two tiles)
+  u32* ticket;       // shared word of the persistent scheduler
+
+  __device__ __forceinline__ void sync() { __syncthreads(); }  // all 128 threads that share the tiles
 
   __device__ __forceinline__ void setup(PairSmem& s, const uint4* __restrict__ bmat) {
-    const u32 tid = threadIdx.x;
+    tid = threadIdx.x;
+    ticket = &s.ticket;
     uint4* sb = reinterpret_cast<uint4*>(s.b);
     for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
     a_row = umma::smem_u32(s.a[0]) + tid * 16u;
@@ -271,11 +276,168 @@ struct PairTile {
     umma::fence_after_sync();
     umma::tmem_ld72_wait(tld, tld + 64u, c);
   }
+  // one half-step: the product in flight -> Z (19 limbs), and the other tile's MMA started as soon as the
+  // accumulator is empty
+  __device__ __forceinline__ void collect(u32 (&z)[20], bool start_next, u32 next) {
+    u32 cols[72];
+    load(cols);
+    if (start_next) start(next);
+    normalise(cols, z);
+  }
 
   __device__ __forceinline__ void teardown() {
     umma::fence_before_sync();
     __syncthreads();
     if (threadIdx.x < 32) umma::tmem_dealloc(tmem, kTmemCols);
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// More accumulators per SM than four (raw advance, cfg2: its 161 instructions per advance leave the tile waiting for
+// the tensor pipe's round trip even with two tiles per accumulator).  Four CTAs of 128 threads fill the SM's 512 TMEM
+// columns with four 128-column allocations although an accumulator needs 80.  So ONE CTA per SM allocates all 512
+// columns and runs kGroups = 6 groups of 128 threads; a group is what a CTA is in PairTile -- two tiles, one accumulator
+// (80 columns at an 80-column stride: measured, an accumulator may start at any multiple of 16 columns), its own A
+// tiles, mbarrier and named barrier -- and the groups never synchronise with each other.  Registers: 65,536 / 768 = 85,
+// so the accumulator is read in three pieces of 24 columns (6 limbs), each normalised before the next is loaded: at
+// most 24 accumulator registers are live instead of 72 (the kernel needs 79).
+constexpr int kGroups = 6;
+constexpr u32 kGroupCols = 80;
+struct GroupSmem {
+  __align__(128) uint8_t a[2][kABytes];
+  __align__(8) u64 bar;
+};
+struct GroupsSmem {
+  __align__(128) uint8_t b[kBBytes];
+  u32 tmem_slot;
+  GroupSmem g[kGroups];
+};
+
+// 24 accumulator columns starting at taddr, then tcgen05.wait::ld -- one asm block, so that no use can be scheduled early
+__device__ __forceinline__ void tmem_ld24_wait(u32 taddr, u32 (&r)[24]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%24];\n\t"
+      "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%16, %17, %18, %19, %20, %21, %22, %23}, [%25];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+        "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+        "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23])
+      : "r"(taddr), "r"(taddr + 16u)
+      : "memory");
+}
+// Piece P of three: columns 24 P .. 24 P + 23 -> limbs 6 P .. 6 P + 5 of Z (see normalise); o_prev = o_(6P-1), cy = the
+// carry of the chain, both handed from piece to piece.
+template <int P>
+__device__ __forceinline__ void normalise_piece(const u32 (&c)[24], u32 (&z)[20], u32& o_prev, u32& cy) {
+  u32 e[6], o[6], t[6];
+#pragma unroll
+  for (int k = 0; k < 6; k++) {
+    e[k] = c[4 * k] + (c[4 * k + 1] << 8);
+    o[k] = c[4 * k + 2] + (c[4 * k + 3] << 8);
+  }
+  t[0] = P == 0 ? o[0] << 16 : __byte_perm(o_prev, o[0], 0x5432);
+#pragma unroll
+  for (int k = 1; k < 6; k++) t[k] = __byte_perm(o[k - 1], o[k], 0x5432);
+  // cy + 0xFFFFFFFF carries out exactly when cy == 1: the chain's carry flag is restored, then saved again
+  asm("{\n\t.reg .u32 scratch;\n\t"
+      "add.cc.u32 scratch, %6, 0xFFFFFFFF;\n\t"
+      "addc.cc.u32 %0, %7, %13;\n\t"
+      "addc.cc.u32 %1, %8, %14;\n\t"
+      "addc.cc.u32 %2, %9, %15;\n\t"
+      "addc.cc.u32 %3, %10, %16;\n\t"
+      "addc.cc.u32 %4, %11, %17;\n\t"
+      "addc.cc.u32 %5, %12, %18;\n\t"
+      "addc.u32 %6, 0, 0;\n\t}"
+      : "=&r"(z[6 * P]), "=&r"(z[6 * P + 1]), "=&r"(z[6 * P + 2]), "=&r"(z[6 * P + 3]), "=&r"(z[6 * P + 4]), "=&r"(z[6 * P + 5]),
+        "+r"(cy)
+      : "r"(e[0]), "r"(e[1]), "r"(e[2]), "r"(e[3]), "r"(e[4]), "r"(e[5]), "r"(t[0]), "r"(t[1]), "r"(t[2]), "r"(t[3]), "r"(t[4]),
+        "r"(t[5]));
+  o_prev = o[5];
+}
+
+struct GroupTile {
+  u32 a_row, bar, phase, tmem, tld, barid;
+  u64 adesc, bdesc;
+  u32 tid;      // thread within the group
+
+  __device__ __forceinline__ void sync() { asm volatile("bar.sync %0, 128;" ::"r"(barid) : "memory"); }
+
+  // CTA-collective (all kGroups x 128 threads)
+  __device__ __forceinline__ void setup(GroupsSmem& s, const uint4* __restrict__ bmat) {
+    const u32 gid = threadIdx.x / kTile;
+    tid = threadIdx.x % kTile;
+    barid = 1u + gid;
+    GroupSmem& g = s.g[gid];
+    uint4* sb = reinterpret_cast<uint4*>(s.b);
+    for (u32 q = threadIdx.x; q < kBBytes / 16; q += kGroups * kTile) sb[q] = __ldg(bmat + q);
+    a_row = umma::smem_u32(g.a[0]) + tid * 16u;
+#pragma unroll
+    for (u32 t = 0; t < 2; t++)
+      asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a_row + t * kABytes + 5u * kAChunk), "r"(0u) : "memory");
+    bar = umma::smem_u32(&g.bar);
+    phase = 0;
+    if (tid == 0) {
+      umma::mbar_init(bar, 1);
+      umma::fence_mbar_init();
+    }
+    if (threadIdx.x < 32) {
+      umma::tmem_alloc(umma::smem_u32(&s.tmem_slot), 512u);
+      umma::tmem_relinquish();
+    }
+    umma::fence_before_sync();
+    __syncthreads();
+    umma::fence_after_sync();
+    tmem = *reinterpret_cast<volatile u32*>(&s.tmem_slot) + gid * kGroupCols;
+    tld = tmem + (((tid >> 5) & 3u) << 21);  // this warp's lane quarter (warp index % 4: groups are whole warpgroups)
+    adesc = umma::smem_desc(umma::smem_u32(g.a[0]), kAChunk, 128u);
+    bdesc = umma::smem_desc(umma::smem_u32(s.b), kBChunk, 128u);
+  }
+  __device__ __forceinline__ void stash(u32 t, const u32 (&x)[18]) {
+    const u32 row = a_row + t * kABytes;
+#pragma unroll
+    for (int g = 0; g < 4; g++)
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(row + (u32)g * kAChunk), "r"(x[4 * g]), "r"(x[4 * g + 1]),
+                   "r"(x[4 * g + 2]), "r"(x[4 * g + 3])
+                   : "memory");
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(row + 4u * kAChunk), "r"(x[16]), "r"(x[17]), "r"(0u) : "memory");
+    umma::fence_proxy_async_smem();
+  }
+  __device__ __forceinline__ void start(u32 t) {
+    umma::fence_before_sync();
+    sync();
+    if (tid < 32) {
+      if (umma::elect_one()) {
+        umma::fence_after_sync();
+        const u64 ad = adesc + (u64)((t * kABytes) >> 4);
+#pragma unroll
+        for (u32 k = 0; k < 3; k++)
+          umma::mma_i8(tmem, ad + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
+        umma::commit(bar);
+      }
+      __syncwarp();
+    }
+  }
+  __device__ __forceinline__ void collect(u32 (&z)[20], bool start_next, u32 next) {
+    umma::mbar_wait(bar, phase);
+    phase ^= 1u;
+    __syncwarp();
+    umma::fence_after_sync();
+    u32 c[24], o_prev = 0, cy = 0;
+    tmem_ld24_wait(tld, c);
+    normalise_piece<0>(c, z, o_prev, cy);
+    tmem_ld24_wait(tld + 24u, c);
+    normalise_piece<1>(c, z, o_prev, cy);
+    tmem_ld24_wait(tld + 48u, c);
+    if (start_next) start(next);  // the accumulator is empty
+    normalise_piece<2>(c, z, o_prev, cy);
+    z[18] = (o_prev >> 16) + cy;
+    z[19] = 0;
+  }
+  // CTA-collective
+  __device__ __forceinline__ void teardown() {
+    umma::fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) umma::tmem_dealloc(tmem, 512u);
   }
 };
 
