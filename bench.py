@@ -30,7 +30,7 @@ IMAD_PER_DOUBLE = 27    # 324 / 12 (one LCG operation per 12 
 # Warp instructions the dominant kernel executes per advance of one warp's 32 streams (ncu smsp__inst_executed.sum /
 # (advances / 32) of the committed --set full captures; profiles/ncu_r02_umma.md).  The issue-slot roofline of the
 # kernels that neither HBM nor the tensor pipe binds: one warp instruction per scheduler and clock.
-WARP_INST_PER_ADVANCE = {"normal": 835, "cfg5": 227, "cfg2": 161}
+WARP_INST_PER_ADVANCE = {"normal": 818, "cfg5": 227, "cfg2": 171}
 TRAFFIC_FILE = "profiles/traffic_r02.json"
 SM_COUNT = 148
 IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles per SMSP, 4 SMSPs
@@ -82,7 +82,7 @@ class ClockSampler:
 
     def __init__(self, cuda_index):
         import threading
-        self.samples = []  # (sm_mhz, power_w, reasons bitmask)
+        self.samples = []  # (time, sm_mhz, power_w, reasons bitmask)
         self.max_mhz = None
         self.err = None
         self._stop = threading.Event()
@@ -115,19 +115,28 @@ class ClockSampler:
                     power = nv.nvmlDeviceGetPowerUsage(self.dev) / 1e3
                 except Exception:
                     power = 0.0
-                self.samples.append((float(mhz), power, int(reasons)))
+                self.samples.append((time.perf_counter(), float(mhz), power, int(reasons)))
             except Exception as e:
                 self.err = repr(e)
                 return
             time.sleep(0.002)
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """Ends the sampling; the summary covers the samples taken in [t0, t1] (perf_counter times; default: all).  The
+        thread is started before the warm-up (the first NVML queries of a process take tens of ms), so a 40 ms timed
+        region still gets its ~20 samples."""
         res = {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0, "source": "nvml"}
         if self._thread is not None:
             self._stop.set()
             self._thread.join(timeout=2)
         if self.err:
             res["error"] = self.err
+        if t0 is not None and self.samples:
+            inside = [x for x in self.samples if t0 <= x[0] <= t1]
+            if not inside:  # region shorter than a sampling period: the sample nearest to it
+                mid = 0.5 * (t0 + t1)
+                inside = [min(self.samples, key=lambda x: abs(x[0] - mid))]
+            self.samples = inside
         if self.samples:
             nv = self.nv
             names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
@@ -135,12 +144,12 @@ class ClockSampler:
                      "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
                      "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
             mask = 0
-            for _, _, r in self.samples:
-                mask |= r
-            sm = sorted(x[0] for x in self.samples)
+            for x in self.samples:
+                mask |= x[3]
+            sm = sorted(x[1] for x in self.samples)
             res.update(sm_mhz=sm[len(sm) // 2], sm_min_mhz=sm[0], samples=len(sm),
                        reasons=sorted(k for k, bit in names.items() if mask & bit),
-                       power_w_max=max(x[1] for x in self.samples))
+                       power_w_max=max(x[2] for x in self.samples))
         return res
 
 
@@ -356,20 +365,22 @@ def main():
         torch.cuda.synchronize()
 
     # ---------------------------------------------------------------- warm-up + timed region
+    sampler = ClockSampler(local) if rank == 0 else None  # started before the warm-up, summarised over the timed region
     for _ in range(args.warmup):
         step()
     barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     launches0 = rlx.rlxpp_launch_count()
     barrier()
+    t_region0 = time.perf_counter()
     ev[0].record(stream)
     for k in range(args.steps):
         step()
         ev[k + 1].record(stream)
     barrier()
+    t_region1 = time.perf_counter()
     launches = rlx.rlxpp_launch_count() - launches0
-    clocks = sampler.stop() if sampler else {}
+    clocks = sampler.stop(t_region0, t_region1) if sampler else {}
     total_ms = ev[0].elapsed_time(ev[-1])
     per_launch_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
     total_ms = shard.max_over_ranks(total_ms, dist, "cuda")
@@ -405,7 +416,7 @@ def main():
                     "frac": alu["frac"], "traffic": None, "peak_source": alu["model"] + f" (DESIGN.md); HBM {peak_src}",
                     "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
     if args.output == "normal":
-        # Box-Muller fused into the emission: 835 warp instructions per advance (ncu, profiles/ncu_r01_umma.md), 342 of
+        # Box-Muller fused into the emission: 818 warp instructions per advance (ncu, profiles/ncu_r02_umma.md), 342 of
         # them fp64: the kernel is bound by instruction issue and the fp64 pipe, not by HBM.  Peak = one warp instruction per scheduler and clock.
         winst = units / 12.0 / 32.0 * WARP_INST_PER_ADVANCE["normal"] / (kernel_ms * 1e-3) / 1e9
         wpeak = SM_COUNT * 4 * sm_max_mhz * 1e6 / 1e9
