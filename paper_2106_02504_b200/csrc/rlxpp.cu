@@ -267,6 +267,7 @@ struct GenArgs {
   u64 n_per;     // draws per stream
   u64 pitch = 0; // STREAM_MAJOR: doubles between the rows of consecutive streams (0 = n_per: dense rows)
   u32 f32_boxes = 0;  // INTERLEAVED floats, aligned: tmap describes the float rows (F32RowStage)
+  u32 ring = 0;       // STREAM_MAJOR, unaligned, even pitch: tmap describes the rows (RingStage)
   double* sum;   // REDUCE: per-stream outputs of this launch (already offset)
   double* sumsq;
   Limbs18 A;
@@ -744,6 +745,90 @@ struct UnalignedRowStage {
   }
 };
 
+// The same case (stream-major, cursors not all at a block boundary) when the row pitch is even, i.e. every row starts
+// 16-byte aligned: the aligned path's store pattern -- boxes of 32 rows handed to the TMA -- survives if the
+// misalignment is moved into shared memory.  Output index q of a row is the same column for all 32 rows of a warp; what
+// differs per lane is only how far it has got: after block step s lane i holds columns up to 12 (s + 1) - pos_i.  So every
+// lane writes its 12 doubles at ITS OWN columns of a ring of three granules (16 doubles = 128 bytes per row, 32 rows:
+// one 4 KB box with SWIZZLE_128B, 2-way bank conflicts at worst), and when the slowest lane (largest cursor of the warp)
+// has completed a granule, lane 0 sends it as one box {16 doubles, 32 rows}.  The lanes are at most 12 doubles apart, so
+// the columns in flight span less than three granules, and the granule written now was sent two steps ago
+// (cp.async.bulk.wait_group.read makes sure it has been read).  Row ends and rows past the launch are clipped by the
+// tensor map: no masked direct stores at all.  12 KB per warp; with the 20 KB of the tile three CTAs per SM.
+constexpr u32 kRingBoxBytes = 32u * 128u;
+constexpr u32 kRingWarpBytes = 3u * kRingBoxBytes;
+constexpr u32 kRingCtaBytes = 4u * kRingWarpBytes + 1024u;  // dynamic shared memory (+ alignment)
+struct RingStage {
+  u32 row;      // shared address of this lane's row in granule slot 0 of its warp's ring
+  u32 rx;       // swizzle term of the row: (lane & 7) << 4
+  u32 p0;       // ring position (0 .. 47) of the first draw of the next block
+  u32 sent;     // granules handed to the TMA (warp-uniform)
+  u32 pmax;     // largest cursor in the warp (warp-uniform): the slowest lane
+  u32 ring;     // shared address of the warp's ring
+  int c1;       // tensor row of the warp's first stream
+  u64 col0;     // tensor column of the item's first draw
+  const void* tmap;
+  u32 kexp;
+  __device__ __forceinline__ void init(uint8_t* stage, const void* tensor_map, u64 tile_first, u64 t0, u32 pos, u32 kexp_) {
+    const u32 lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    ring = ((umma::smem_u32(stage) + 1023u) & ~1023u) + warp * kRingWarpBytes;
+    row = ring + lane * 128u;
+    rx = (lane & 7u) << 4;
+    p0 = pos ? 48u - pos : 0u;  // block 0 starts pos columns before the item's first draw
+    sent = 0;
+    pmax = __reduce_max_sync(0xFFFFFFFFu, pos);
+    c1 = (int)(tile_first + warp * 32u);
+    col0 = t0;
+    tmap = tensor_map;
+    kexp = kexp_;
+  }
+  // shared address of ring position p (0 .. 47) of this lane's row: slot p / 16, 16-byte chunk (p % 16) / 2 XOR-swizzled
+  // with the row, half p % 2
+  __device__ __forceinline__ u32 at(u32 p) const {
+    const u32 ps = p << 3;
+    return row + ((ps & 0x180u) << 5) + ((ps & 0x78u) ^ rx);
+  }
+  template <int OUT, int J, bool MASKED>
+  __device__ __forceinline__ void put(const u32 (&v)[18], u64 q0, u64 n) {
+    if constexpr (J < 12) {
+      double a, b;
+      draw_pair<OUT, J>(v, kexp, a, b);
+      u32 pa = p0 + J, pb = p0 + J + 1;
+      pa = pa >= 48u ? pa - 48u : pa;
+      pb = pb >= 48u ? pb - 48u : pb;
+      if (!MASKED || q0 + J < n) asm volatile("st.shared.f64 [%0], %1;" ::"r"(at(pa)), "d"(a) : "memory");
+      if (!MASKED || q0 + J + 1 < n) asm volatile("st.shared.f64 [%0], %1;" ::"r"(at(pb)), "d"(b) : "memory");
+      put<OUT, J + 2, MASKED>(v, q0, n);
+    }
+  }
+  // whole-warp call: block step s (0 = the current block).  Draw j of the block is output index q = 12 s + j - pos of the
+  // item if that is in [0, n) (it wraps below zero for draws before the cursor: then q >= n).
+  template <int OUT, bool MASKED>
+  __device__ __forceinline__ void emit(const u32 (&v)[18], u64 s, u32 pos, u64 n) {
+    if ((threadIdx.x & 31u) == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    __syncwarp();
+    put<OUT, 0, MASKED>(v, 12 * s - pos, n);
+    p0 = p0 + 12u >= 48u ? p0 - 36u : p0 + 12u;
+    umma::fence_proxy_async_smem();
+    __syncwarp();
+    // granules every lane has completed: the slowest lane holds columns up to 12 (s + 1) - pmax
+    const u64 have = 12 * (s + 1) >= pmax ? 12 * (s + 1) - pmax : 0;
+    const u32 done = (u32)(have >= n ? (n + 15) / 16 : have / 16);
+    if ((threadIdx.x & 31u) == 0 && done > sent) {
+      for (u32 g = sent; g < done; g++)
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap),
+                     "r"((int)(col0 + 16ull * g)), "r"(c1), "r"(ring + (g % 3u) * kRingBoxBytes)
+                     : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    sent = done > sent ? done : sent;
+  }
+  __device__ __forceinline__ void drain() {  // before the ring serves another item or the CTA exits
+    if ((threadIdx.x & 31u) == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    __syncwarp();
+  }
+};
+
 // Interleaved 24-bit floats (rlxpp_generate_floats, aligned cursors).  A float row holds 4 bytes per stream: direct
 // stores are 24 instructions of 128 bytes per warp and advance (measured 700 G draws/s).  Instead the CTA parks a
 // block as [24 float rows][128 streams] in shared memory and ONE thread of the MMA-issuing warp hands it to the TMA
@@ -834,9 +919,9 @@ template <int MODE, bool ALIGNED, int OUT = kF64>
 __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(const __grid_constant__ GenArgs a) {
   __shared__ tc::Smem smem;
   constexpr bool kStaged = MODE == kStoreStreamMajor && ALIGNED;
-  extern __shared__ __align__(128) uint8_t stage[];  // kStageCtaBytes when kStaged, else none
+  extern __shared__ __align__(128) uint8_t stage[];  // kStageCtaBytes when kStaged; float row boxes; row stage or ring; else none
   constexpr bool kRowStaged = MODE == kStoreStreamMajor && !ALIGNED;
-  __shared__ __align__(16) uint8_t row_stage[kRowStaged ? 4 * kRowStageWarpBytes : 16];
+  const bool ring = kRowStaged && a.ring != 0;
   tc::Tile<MODE == kReduce ? tc::kSyncCta : tc::kSyncArrive> tile;
   tile.setup(smem, a.bmat);
   // the parameter form saves 12 instructions per advance and helps the ALU-bound fused kernel (+5 %); the
@@ -913,16 +998,21 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
       const u64 last = ((u64)pos + (n - 1)) / 12;  // own last block
       const u64 smax = (12 + (n - 1)) / 12;        // last block of any thread (uniform)
       UnalignedRowStage rs;
+      RingStage rg;
       if (kRowStaged) {
 #pragma unroll
         for (int j = 0; j < 18; j++) v[j] = 0;  // lanes without a current block still take part in the warp's copy
-        rs.init(row_stage, a.out + t0, (u64)tidx * tc::kTile + (threadIdx.x & ~31u), a.count, pitch, kexp);
+        if (ring) rg.init(stage, &a.tmap, (u64)tidx * tc::kTile, t0, pos, kexp);
+        else rs.init(stage, a.out + t0, (u64)tidx * tc::kTile + (threadIdx.x & ~31u), a.count, pitch, kexp);
       }
       if (pos < 12) {
         to_ranlux_exact(x, v, c);
         if (!kRowStaged && live) EmitBlock<0, MODE, OUT>::masked(sink, v, 0, pos, n);
       }
-      if (kRowStaged) rs.emit<OUT>(v, 0, pos, n);  // cursor 12: every position lies before the cursor, nothing is stored
+      if (kRowStaged) {  // cursor 12: every position lies before the cursor, nothing is stored
+        if (ring) rg.emit<OUT, true>(v, 0, pos, n);
+        else rs.emit<OUT>(v, 0, pos, n);
+      }
       tile.issue(x);
       // blocks 1 .. smax - 2 lie wholly inside [0, n) for every cursor (last >= smax - 1): no masks
       u64 s = 1;
@@ -933,8 +1023,10 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
         tc::reduce_z(z, x);
         tile.issue(x);
         to_ranlux_hot(x, v, c);
-        if (kRowStaged) rs.emit<OUT>(v, s * 12, pos, n);
-        else if (live) EmitBlock<0, MODE, OUT>::template all<false>(sink, v, s * 12 - pos);
+        if (kRowStaged) {
+          if (ring) rg.emit<OUT, false>(v, s, pos, n);
+          else rs.emit<OUT>(v, s * 12, pos, n);
+        } else if (live) EmitBlock<0, MODE, OUT>::template all<false>(sink, v, s * 12 - pos);
       }
 #pragma unroll 1
       for (; s <= smax; s++) {
@@ -951,8 +1043,12 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_kernel(
           to_ranlux_hot(x, v, c);
           if (!kRowStaged && live) EmitBlock<0, MODE, OUT>::masked(sink, v, s * 12, pos, n);
         }
-        if (kRowStaged) rs.emit<OUT>(v, s * 12, pos, n);  // a stream that ended a block early has all of it past n
+        if (kRowStaged) {  // a stream that ended a block early has all of it past n
+          if (ring) rg.emit<OUT, true>(v, s, pos, n);
+          else rs.emit<OUT>(v, s * 12, pos, n);
+        }
       }
+      if (ring) rg.drain();
       pos = (u32)((u64)pos + n - 12 * last);
     }
     if (live) {
@@ -1788,6 +1884,22 @@ static int encode_f32_rows_map(CUtensorMap* map, float* out, uint64_t count, uin
   return RLXPP_OK;
 }
 
+// Tensor map of a stream-major output whose rows are written through RingStage (cursors not at a block boundary):
+// out[count][n_per] doubles with a row pitch of `pitch` doubles (even), box = 16 doubles x 32 rows, 128-byte swizzle.
+static int encode_ring_map(CUtensorMap* map, double* out, uint64_t count, uint64_t n_per, uint64_t pitch) {
+  TensorMapEncodeFn encode = nullptr;
+  const int erc = tensor_map_encoder(&encode);
+  if (erc) return erc;
+  const cuuint64_t dims[2] = {n_per, count};
+  const cuuint64_t strides[1] = {pitch * sizeof(double)};
+  const cuuint32_t box[2] = {16, 32};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, out, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(RLXPP_ECUDA, "cuTensorMapEncodeTiled (ring rows) failed (%d)", (int)r);
+  return RLXPP_OK;
+}
+
 template <int MODE, int OUT = kF64>
 static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   if (MODE == kStoreInterleaved && OUT == kF32 && aligned && a.ld % 4 == 0 && a.count < (1ull << 31) && a.n_per < (1ull << 30)) {
@@ -1803,7 +1915,12 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   // tiles.  (Interleaved floats keep the one-tile kernel with its row boxes, stream-major its staged TMA path.)
   constexpr bool kPairs = MODE == kReduce || (MODE == kStoreInterleaved && OUT != kF32);
   const uint64_t n_tiles = kPairs ? (a.count + 2 * tc::kTile - 1) / (2 * tc::kTile) : (a.count + tc::kTile - 1) / tc::kTile;
-  const unsigned slots = tc_slots();
+  // stream-major rows shifted against each other go through per-lane rings and TMA boxes when the rows are 16-byte
+  // aligned (even pitch; RingStage: 69 KB of shared memory, three CTAs per SM), else through the warp's row stage
+  const uint64_t row_pitch = a.pitch ? a.pitch : a.n_per;
+  const bool ring = MODE == kStoreStreamMajor && !aligned && row_pitch % 2 == 0 && (uintptr_t)a.out % 16 == 0 &&
+                    a.count < (1ull << 31) && a.n_per < (1ull << 31);
+  const unsigned slots = ring ? tc_slots() / tc::kCtasPerSm * 3 : tc_slots();
   a.n_tiles = (u32)n_tiles;
   if constexpr (MODE != kReduce) {
     // Short calls that leave most of the grid empty: K lanes per tile, each reaching its blocks with the matrices of
@@ -1844,6 +1961,18 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
       if (rc) return rc;
     }
     tc_generate_kernel<MODE, true, OUT><<<grid, tc::kTile, kStaged ? kStageCtaBytes : (a.f32_boxes ? kF32StageBytes : 0), s>>>(a);
+  } else if (MODE == kStoreStreamMajor) {
+    unsigned dyn = 4 * kRowStageWarpBytes;
+    if (ring) {
+      int rc = encode_ring_map(&a.tmap, a.out, a.count, a.n_per, row_pitch);
+      if (rc) return rc;
+      static std::atomic<uint64_t> done{0};  // 20 KB static + 49 KB of rings: three CTAs per SM
+      rc = allow_dynamic_smem(tc_generate_kernel<MODE, false, OUT>, done, (int)kRingCtaBytes);
+      if (rc) return rc;
+      a.ring = 1;
+      dyn = kRingCtaBytes;
+    }
+    tc_generate_kernel<MODE, false, OUT><<<grid, tc::kTile, dyn, s>>>(a);
   } else {
     tc_generate_kernel<MODE, false, OUT><<<grid, tc::kTile, 0, s>>>(a);
   }

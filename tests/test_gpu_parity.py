@@ -1032,3 +1032,52 @@ def test_short_calls_run_time_parallel(rlx, torch, oracle, nthreads, n, blocks):
             assert_within_ulps(got, oracle.normals(ints), NORMAL_ULPS, what)
     check_state(rlx, torch, h, ref, "after time-parallel calls")
     rlx.rlxpp_destroy(h)
+
+
+@pytest.mark.parametrize("per, n_chunks", [(2, 0), (30, 0), (96, 0), (250, 0), (1536, 0), (12 * 50 + 6, 3), (251, 0)])
+def test_stream_major_per_stream_cursors_through_rings(rlx, torch, oracle, nthreads, per, n_chunks):
+    """Stream-major output when the cursors are not at a block boundary (per-stream skips; one odd common cursor).  UMMA
+    engine, even row length: every lane writes its 12 doubles at its own columns of a shared-memory ring and the warp sends
+    128-byte granules of 32 rows as TMA boxes once its slowest lane has completed them (rlxpp.cu RingStage); row ends and
+    rows past the launch are clipped by the tensor map.  Rows of 2 doubles up to cfg3's 1,536, a length that is not a
+    multiple of 16, forced chunks (granule-aligned item starts), a ragged last tile, all 8-byte output forms, the guard
+    band behind the buffer, two calls in a row; per = 251 (odd pitch) takes the element-wise row stage instead."""
+    n = 3 * 128 + 45
+    dist = inputs.splitmix64(777, n) % np.uint64(40)  # every cursor value occurs
+    ref = oracle.streams(inputs.seeds(n, 17), 2048, 3 * per + 2, skips=dist, want=("ints", "doubles", "state"), nthreads=nthreads)
+    h = rlx.rlxpp_create(n, 17, 2048)
+    rlx.rlxpp_skip_each(h, torch.from_numpy(dist.view(np.int64)).cuda())
+    rlx.rlxpp_set_chunks(n_chunks)
+    try:
+        at = 0
+        for form in ("doubles", "u48", "doubles"):
+            buf = torch.full((n * per + 512,), -1.0, dtype=torch.float64, device="cuda")
+            if form == "doubles":
+                rlx.rlxpp_generate_doubles(h, buf, per, rlx.RLXPP_STREAM_MAJOR)
+            else:
+                rlx.rlxpp_generate_u48(h, buf.view(torch.int64), per, rlx.RLXPP_STREAM_MAJOR)
+            torch.cuda.synchronize()
+            raw = buf.cpu().numpy()
+            assert np.all(raw[n * per:] == -1.0), "wrote behind the output buffer"
+            got = raw[:n * per].reshape(n, per)
+            what = f"per-stream cursors, rows of {per}, {form}, draws {at}..{at + per}"
+            if form == "doubles":
+                assert_bits_equal(got, ref["doubles"][:, at:at + per], what)
+            else:
+                assert np.array_equal(got.view(np.uint64), ref["ints"][:, at:at + per]), what
+            at += per
+    finally:
+        rlx.rlxpp_set_chunks(0)
+    # normal deviates from the same cursors (pairs counted from each stream's first draw)
+    z = torch.full((n, per + (per & 1)), np.nan, dtype=torch.float64, device="cuda")
+    per_n = per + (per & 1)
+    rlx.rlxpp_generate_normal(h, z, per_n, rlx.RLXPP_STREAM_MAJOR)
+    g = dist + np.uint64(at)
+    odd = (g & np.uint64(1)).astype(np.int64)
+    k = oracle.streams(inputs.seeds(n, 17), 2048, per_n + 2, skips=g - odd.astype(np.uint64), want=("ints",), nthreads=nthreads)["ints"]
+    zz = oracle.normals(k)
+    want = np.stack([zz[i, odd[i]:odd[i] + per_n] for i in range(n)])
+    assert_within_ulps(z.cpu().numpy(), want, NORMAL_ULPS, f"normals through rings, rows of {per_n}")
+    ref2 = oracle.streams(inputs.seeds(n, 17), 2048, 0, skips=g + np.uint64(per_n), want=("state",), nthreads=nthreads)
+    check_state(rlx, torch, h, ref2, "after ring calls")
+    rlx.rlxpp_destroy(h)
