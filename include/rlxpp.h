@@ -11,7 +11,10 @@
  * numbers of 24 bits + carry, sec. 2/2.3).  One LCG advance is
  * X <- A X mod m with A = a^p mod m, p the luxury level;
  * each advance yields 12 doubles k 2^-48, k = 48 consecutive bits of V.
- * A fresh stream has pos = 12, i.e. the first draw advances first (D8, c-6).
+ * A fresh stream has pos = 12, i.e. the first draw advances first (D8, c-6).  The paper does not say whether the
+ * block of the seeded state itself is emitted (parity with the published engine unpinned): an engine
+ * that starts at pos = 0 produces this library's sequence with one extra leading block, and
+ * rlxpp_set_state(rlxpp_seed_state(seed, p), pos = 0) starts a stream there.
  *
  * Conventions.
  *   - Every function returns 0 on success and a negative RLXPP_E* code on error;

@@ -28,6 +28,7 @@
 // The next issue() orders the TMEM reads before the next MMA's TMEM writes (fence + barrier),
 // and the mbarrier wait orders the MMA's shared-memory reads before the next A-tile stores.
 #pragma once
+#include "arith.cuh"
 #include "umma.cuh"
 
 namespace rlx {
