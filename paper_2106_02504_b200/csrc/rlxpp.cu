@@ -650,10 +650,6 @@ int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, ui
     const uint4* bmat = nullptr;
     rc = get_bmatrix(p, &bmat);
     if (rc) return rc;
-    const uint64_t tiles = (n_states + tc::kTile - 1) / tc::kTile;
-    // one CTA per tile: measured faster than a persistent grid here (1,050 vs 946 G doubles-equivalent/s at
-    // cfg2: with 16 advances per tile the load / compute / store phases of co-resident CTAs overlap better when
-    // the CTAs are not in lock step); the kernel's tile loop serves grids smaller than the tile count
     {  // one CTA per SM with tc::kGroups groups (cfg2: 1,180 with pairs in four CTAs, 1,228 with 5 groups, 1,320 with 6)
       const size_t smem_bytes = ((sizeof(tc::GroupsSmem) + 127) & ~(size_t)127) +
                                 (layout == RLXPP_AOS ? (size_t)tc::kGroups * kRawStageWords * sizeof(uint4) : 0);

@@ -405,6 +405,8 @@ struct GroupTile {
   }
   __device__ __forceinline__ void start(u32 t) {
     umma::fence_before_sync();
+    // (all 128 threads bar.sync: the group's barrier also serves the raw state staging, so an arrive-and-run-on
+    // hand-off as in PairTile could count a warp twice in one phase)
     sync();
     if (tid < 32) {
       if (umma::elect_one()) {
