@@ -219,78 +219,6 @@ __device__ __forceinline__ void normalise(const u32 (&c)[72], u32 (&z)[20]) {
 
 }  // namespace tile
 
-// ---------------------------------------------------------------------------------------------------- fast forms
-// mod_m and to_ranlux as the hot paths run them: the overwhelmingly likely case, a `rare` flag otherwise;
-// the caller then recomputes with the exact functions of rlxpp_device.cuh (mod_m20, to_ranlux_exact).
-namespace detail {
-
-// Fast fold of z (20 limbs, hi = z[18] + z[19] 2^32 < 2^37) to x = z mod 2^576 - hi + hi 2^240.
-// Exact iff `rare` stays 0:  rare is raised when the borrow of "- hi" leaves limb 1, when the
-// carry of "+ hi 2^240" leaves limb 9, or when the top limb is all ones (x might be >= m).
-__device__ __forceinline__ void fold_fast(const u32 (&z)[20], u32 (&x)[18], u32& rare) {
-  const u32 h0 = z[18], h1 = z[19];
-  const u32 s0 = h0 << 16;
-  const u32 s1 = __funnelshift_l(h0, h1, 16);  // bits 16..47 of hi
-  const u32 s2 = h1 >> 16;
-  u32 brw, cry;
-  asm("sub.cc.u32 %0, %3, %5;\n\t"
-      "subc.cc.u32 %1, %4, %6;\n\t"
-      "subc.u32 %2, 0, 0;"
-      : "=r"(x[0]), "=r"(x[1]), "=r"(brw)
-      : "r"(z[0]), "r"(z[1]), "r"(h0), "r"(h1));
-  asm("add.cc.u32 %0, %4, %7;\n\t"
-      "addc.cc.u32 %1, %5, %8;\n\t"
-      "addc.cc.u32 %2, %6, %9;\n\t"
-      "addc.u32 %3, 0, 0;"
-      : "=r"(x[7]), "=r"(x[8]), "=r"(x[9]), "=r"(cry)
-      : "r"(z[7]), "r"(z[8]), "r"(z[9]), "r"(s0), "r"(s1), "r"(s2));
-#pragma unroll
-  for (int j = 2; j < 7; j++) x[j] = z[j];
-#pragma unroll
-  for (int j = 10; j < 18; j++) x[j] = z[j];
-  // borrow out of limb 1 is harmless only if it is absorbed below limb 7: we do not track
-  // that here -- any borrow or carry goes to the exact path.
-  rare |= brw | cry | (x[17] == 0xFFFFFFFFu ? 1u : 0u);
-}
-
-// Fast to_ranlux.  With u = bits 304..335 of X and w = bits 544..575 of X (the leading
-// 32 bits of the middle and of the top 240-bit field):
-//   u >= w + 2 and u != 2^32 - 1  =>  D > 0, no overflow of Xl + Xh:  V = X + Xh,     c = 0
-//   u + 2 <= w                    =>  D < 0:                          V = X + Xh - 1, c = 1
-// (derivation in DESIGN.md).  Otherwise, or if the 8-limb addition carries out of limb 7,
-// or if the "- c" would borrow, `rare` is raised.  Limbs 8..17 of V equal those of X.
-__device__ __forceinline__ void to_ranlux_fast(const u32 (&x)[18], u32 (&v)[18], u32& c_out, u32& rare) {
-  const u32 u = __funnelshift_r(x[9], x[10], 16);
-  const u32 w = x[17];
-  const u32 c = u < w ? 1u : 0u;
-  const u32 d = u - w + 1u;  // in {0, 1, 2}  <=>  |u - w| <= 1
-  u32 xh[8];
-#pragma unroll
-  for (int j = 0; j < 7; j++) xh[j] = __funnelshift_r(x[10 + j], x[11 + j], 16);
-  xh[7] = x[17] >> 16;
-  u32 cry;
-  asm("add.cc.u32 %0, %9, %17;\n\t"
-      "addc.cc.u32 %1, %10, %18;\n\t"
-      "addc.cc.u32 %2, %11, %19;\n\t"
-      "addc.cc.u32 %3, %12, %20;\n\t"
-      "addc.cc.u32 %4, %13, %21;\n\t"
-      "addc.cc.u32 %5, %14, %22;\n\t"
-      "addc.cc.u32 %6, %15, %23;\n\t"
-      "addc.cc.u32 %7, %16, %24;\n\t"
-      "addc.u32 %8, 0, 0;"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(cry)
-      : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(x[7]), "r"(xh[0]),
-        "r"(xh[1]), "r"(xh[2]), "r"(xh[3]), "r"(xh[4]), "r"(xh[5]), "r"(xh[6]), "r"(xh[7]));
-  rare |= cry | (d <= 2u ? 1u : 0u) | (u == 0xFFFFFFFFu ? 1u : 0u) | (v[0] < c ? 1u : 0u);
-  v[0] -= c;
-#pragma unroll
-  for (int j = 8; j < 18; j++) v[j] = x[j];
-  c_out = c;
-}
-
-}  // namespace detail
-
-
 // ---------------------------------------------------------------------------------------------------- TileStream
 // Shared memory of one CTA of 128 threads (declare it __shared__ in the kernel; 44 KB).
 struct alignas(128) TileShared {

@@ -392,13 +392,31 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     // readers): n_tiles K <= slots.  rlxpp_set_chunks(c > 0) keeps the persistent path.
     const uint64_t nblk = a.n_per / 12, tiles1 = (a.count + tc::kTile - 1) / tc::kTile;  // lanes work on single tiles
     uint64_t K = nblk < kMaxLanes ? nblk : kMaxLanes;
-    if (K > slots / tiles1) K = slots / tiles1;
+    uint64_t lane_slots = slots;
+    if (aligned && a.lane_sync && g_force_chunks.load() == 0 && K >= 4 && tiles1 * 4 <= slots) {
+      // what the runtime will accept as a cooperative grid: queried once per (kernel, device)
+      static std::atomic<int> cached[64];
+      int dev = 0, per_sm = 0;
+      CUDA_TRY(cudaGetDevice(&dev));
+      if (dev < 64) per_sm = cached[dev].load();
+      if (per_sm == 0) {
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc_generate_lanes_kernel<MODE, OUT>, tc::kTile, 0));
+        if (dev < 64) cached[dev].store(per_sm);
+      }
+      lane_slots = (uint64_t)(slots / tc::kCtasPerSm) * (uint64_t)(per_sm < tc::kCtasPerSm ? per_sm : tc::kCtasPerSm);
+    }
+    if (K > lane_slots / tiles1) K = lane_slots / tiles1;
     if (aligned && a.lane_sync && K >= 4 && g_force_chunks.load() == 0) {
       int rc = get_bmatrix_powers(a.p, &a.bmat_pow);
       if (rc) return rc;
       a.lanes = (u32)K;
-      tc_generate_lanes_kernel<MODE, OUT><<<(unsigned)(tiles1 * K), tc::kTile, 0, s>>>(a);
-      LAUNCH_CHECK();
+      // A cooperative launch: the lane that writes a tile's new state waits for the tile's other lanes to have read the
+      // old one, so all CTAs must be resident together -- the runtime guarantees it (and holds the launch back while other
+      // work occupies the SMs) instead of the grid size merely allowing it.
+      void* params[] = {&a};
+      CUDA_TRY(cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(&tc_generate_lanes_kernel<MODE, OUT>),
+                                           dim3((unsigned)(tiles1 * K)), dim3(tc::kTile), params, 0, s));
+      g_launches++;
       return RLXPP_OK;
     }
   }
