@@ -401,8 +401,9 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_pair_kernel(cons
 // Raw advance (cfg2; S8 a-3 / a-4 alone): x <- A^reps x on raw uint64[9] states, in place.  Two tiles per accumulator
 // (the other tile's MMA runs under this tile's normalisation, as in tc_pair_kernel) and tc::kGroups groups of 128
 // threads in one CTA per SM (tc::GroupTile): six accumulators per SM instead of four.  Persistent: group (CTA c, group g)
-// strides over the pairs of tiles.  Measured at cfg2 (G doubles-equivalent/s): one tile per CTA 1,160; pairs in four
-// CTAs 1,180; 5 groups 1,228; 6 groups 1,320.
+// strides over the pairs of tiles.  Between repetitions the state stays an UNREDUCED product (19 limbs): mod_m is
+// linear-algebra-free to defer because A z == A (z mod m), so only the last repetition pays the fold.  Measured at cfg2
+// (G doubles-equivalent/s): one tile per CTA 1,160; pairs in four CTAs 1,180; 5 groups 1,228; 6 groups 1,320.
 struct GroupSync {
   u32 barid;
   __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 128;" ::"r"(barid) : "memory"); }
@@ -444,11 +445,17 @@ __global__ void __launch_bounds__(tc::kGroups * tc::kTile, 1) tc_advance_states_
       for (int t = 0; t < 2; t++) {
         u32 z[20];
         tile.collect(z, t == 0 || r + 1 < reps, t ^ 1);
-        tc::reduce_z(z, x);
-        if (r + 1 < reps) tile.stash(t, x);
-        else if (2 * pair + t < n_tiles) {
-          store_raw<LAYOUT>(states, n, stage, x, 2 * pair + t, tile.tid, gsync);
-          gsync();
+        if (r + 1 < reps) {
+          // mod_m deferred: the product (< 2^591) is the next operand as it is -- the byte matrix has columns for
+          // its two bytes above 2^576 (A z == A (z mod m); the next product is < 2^591 again) -- and only the last
+          // repetition is folded to the canonical value ("smaller than m in all cases")
+          tile.stash19(t, z);
+        } else {
+          tc::reduce_z(z, x);
+          if (2 * pair + t < n_tiles) {
+            store_raw<LAYOUT>(states, n, stage, x, 2 * pair + t, tile.tid, gsync);
+            gsync();
+          }
         }
       }
     }

@@ -114,7 +114,7 @@ static const Tables& cached_tables(uint32_t p) {
 static void build_bmatrix(uint32_t p, std::vector<uint8_t>& img) {
   img.assign(tc::kBBytes, 0);
   host::Big R = host::multiplier_ap(p);
-  for (int k = 0; k < 72; k++) {
+  for (int k = 0; k < tc::kKUsed; k++) {  // 72 bytes of a state + the two bytes an unreduced product has above 2^576
     uint32_t w[18];
     R.to_u32x18(w);
     for (int n = 0; n < 72; n++) img[tc::b_offset(n, k)] = (uint8_t)(w[n / 4] >> (8 * (n % 4)));
@@ -160,7 +160,7 @@ static int get_bmatrix_powers(uint32_t p, const uint4** out) {
   for (u32 k = 0; k < kMaxLanes; k++) {
     host::Big R = R0;
     uint8_t* img = all.data() + (size_t)k * tc::kBBytes;
-    for (int col = 0; col < 72; col++) {
+    for (int col = 0; col < tc::kKUsed; col++) {
       uint32_t w[18];
       R.to_u32x18(w);
       for (int n = 0; n < 72; n++) img[tc::b_offset(n, col)] = (uint8_t)(w[n / 4] >> (8 * (n % 4)));

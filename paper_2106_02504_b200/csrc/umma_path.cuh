@@ -46,6 +46,9 @@ using rlxpp_dev::tile::kCtasPerSm;
 using rlxpp_dev::tile::kIdesc;
 using rlxpp_dev::tile::b_offset;
 using rlxpp_dev::tile::normalise;
+// K columns of the byte matrix that are filled: the 72 bytes of a state, and bytes 72, 73 for operands that are products
+// not yet folded (Z < 2^591: the raw advance keeps its state unreduced between repetitions, GroupTile::stash19)
+constexpr int kKUsed = 74;
 
 // How the CTA hands the freshly written A tile to the thread that issues the MMAs.
 //   kSyncCta:    __syncthreads, warp 0 issues.  Every warp waits for the slowest one.
@@ -401,6 +404,18 @@ struct GroupTile {
                    "r"(x[4 * g + 2]), "r"(x[4 * g + 3])
                    : "memory");
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(row + 4u * kAChunk), "r"(x[16]), "r"(x[17]), "r"(0u) : "memory");
+    umma::fence_proxy_async_smem();
+  }
+  // the same for an unreduced product z (19 limbs, z[18] < 2^15): A z == A (z mod m), so the fold can wait
+  __device__ __forceinline__ void stash19(u32 t, const u32 (&z)[20]) {
+    const u32 row = a_row + t * kABytes;
+#pragma unroll
+    for (int g = 0; g < 4; g++)
+      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(row + (u32)g * kAChunk), "r"(z[4 * g]), "r"(z[4 * g + 1]),
+                   "r"(z[4 * g + 2]), "r"(z[4 * g + 3])
+                   : "memory");
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(row + 4u * kAChunk), "r"(z[16]), "r"(z[17]), "r"(z[18]), "r"(0u)
+                 : "memory");
     umma::fence_proxy_async_smem();
   }
   __device__ __forceinline__ void start(u32 t) {

@@ -59,14 +59,16 @@ def rlx(torch, engine):
 
 
 # ------------------------------------------------------------------------------------- the model of the decisions
-R_BYTE = [(A << (8 * k)) % M for k in range(72)]    # UMMA engine: rows of the byte matrix
+R_BYTE = [(A << (8 * k)) % M for k in range(74)]    # UMMA engine: rows of the byte matrix; rows 72, 73
+                                                    # serve operands that are unreduced products (< 2^591: raw advance)
 R_LIMB = [(A << (32 * i)) % M for i in range(18)]   # IMAD engine: pre-reduced rows
 
 
 def product(engine, x):
     """The unreduced value z == A x (mod m) the engine's multiply leaves for fold_fast."""
     if engine == "umma":
-        return sum(((x >> (8 * k)) & 0xFF) * R_BYTE[k] for k in range(72))
+        assert x < 1 << 592
+        return sum(((x >> (8 * k)) & 0xFF) * R_BYTE[k] for k in range(74))
     return sum(((x >> (32 * i)) & MASK32) * R_LIMB[i] for i in range(18))
 
 
@@ -419,7 +421,9 @@ def test_rare_branches_unaligned(rlx, torch, oracle, engine, mode, cursors):
 @pytest.mark.parametrize("layout", ["aos", "soa"])
 def test_rare_branches_raw_advance(rlx, torch, oracle, engine, layout):
     """rlxpp_advance_states (cfg2's kernel): only the fold.  Besides the pre-images, raw non-canonical inputs with the
-    largest products: 2^576 - 1 (all bytes 0xFF: the largest z[18] the byte products can give), m, m + 1."""
+    largest products: 2^576 - 1 (all bytes 0xFF: the largest z[18] the byte products can give), m, m + 1.  The UMMA
+    kernel folds only the last of the `reps` products (the state stays an unreduced product in between), so the crafted
+    state must be the FINAL one to reach its fold: depth d = reps."""
     reps = 4
     x0s, info = build_streams(3 * 128 + 61, (1, 2, 3, 4))
     x0s = x0s + [FULL, M, M + 1, FULL - 1, M - 2]
@@ -438,8 +442,20 @@ def test_rare_branches_raw_advance(rlx, torch, oracle, engine, layout):
     assert np.array_equal(got, want), f"raw advance {layout}"
     for i, x in enumerate(x0s):  # and against Python itself
         assert inputs.limbs_to_int(got[i]) == pow(A, reps, M) * x % M
-    assert_counts(rlx, model_counts(engine, oracle, x0s, [reps] * n, [0] * n), f"raw advance {layout}",
-                  (BORROW, CARRY, TOP))
+    if engine == "umma":
+        # the tensor-core raw advance keeps the state UNREDUCED between repetitions (the byte matrix has columns for
+        # the two bytes above 2^576) and folds the last product only: one fold per state, of the reps-fold product chain
+        want_counts = np.zeros(8, np.uint64)
+        for x in x0s:
+            z = x
+            for _ in range(reps):
+                z = product("umma", z)
+            assert z % M == pow(A, reps, M) * x % M and z < 1 << 591
+            for k in range(8):
+                want_counts[k] += (fold_mask(z) >> k) & 1
+    else:
+        want_counts = model_counts(engine, oracle, x0s, [reps] * n, [0] * n)
+    assert_counts(rlx, want_counts, f"raw advance {layout}", (BORROW, CARRY, TOP))
     # the largest overflow limb: z >> 576 for the all-ones input, as the model computes it
     assert 8000 < product("umma", FULL) >> 576 < 1 << 15 and product("imad", FULL) >> 576 < 1 << 37
 
