@@ -587,6 +587,7 @@ def main():
         e2e = {"value": units * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": args.e2e_steps,
                "per_step_this_rank": {"min": each["min"], "median": each["median"], "max": each["max"], "unit": UNIT},
+               "d2h_gb_per_s_median_step": d2h * each["median"] / units / 1e9,  # what binds it: the PCIe copy of the result
                "what": "rlxpp_create (seed kernel) + rlxpp_generate_*_host into pinned host memory + rlxpp_destroy, wall clock"}
 
     # ---------------------------------------------------------------- oracle on the host cores
