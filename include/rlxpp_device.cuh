@@ -383,6 +383,43 @@ __device__ __forceinline__ void to_ranlux_exact(const u32 (&x)[18], u32 (&v)[18]
 }
 
 // ------------------------------------------------------------------ hot-path fast forms
+// Row-reduced product of a FIXED multiplier (include/rlxpp_rows.cuh): Z = sum_i x_i R_i < 2^613 arrives as two
+// interleaved sets of 64-bit accumulators E / O; merge_eo adds them into 20 limbs.
+__device__ __forceinline__ void merge_eo(const u64 (&E)[9], u32 e9, const u64 (&O)[9], u32 o9, u32 (&z)[20]) {
+  u32 el[19], ol[19];
+#pragma unroll
+  for (int w = 0; w < 9; w++) {
+    el[2 * w] = (u32)E[w];
+    el[2 * w + 1] = (u32)(E[w] >> 32);
+    ol[2 * w] = (u32)O[w];
+    ol[2 * w + 1] = (u32)(O[w] >> 32);
+  }
+  el[18] = e9;
+  ol[18] = o9;
+  z[0] = el[0];
+  asm("add.cc.u32 %0, %19, %37;\n\t"
+      "addc.cc.u32 %1, %20, %38;\n\t"
+      "addc.cc.u32 %2, %21, %39;\n\t"
+      "addc.cc.u32 %3, %22, %40;\n\t"
+      "addc.cc.u32 %4, %23, %41;\n\t"
+      "addc.cc.u32 %5, %24, %42;\n\t"
+      "addc.cc.u32 %6, %25, %43;\n\t"
+      "addc.cc.u32 %7, %26, %44;\n\t"
+      "addc.cc.u32 %8, %27, %45;\n\t"
+      "addc.cc.u32 %9, %28, %46;\n\t"
+      "addc.cc.u32 %10, %29, %47;\n\t"
+      "addc.cc.u32 %11, %30, %48;\n\t"
+      "addc.cc.u32 %12, %31, %49;\n\t"
+      "addc.cc.u32 %13, %32, %50;\n\t"
+      "addc.cc.u32 %14, %33, %51;\n\t"
+      "addc.cc.u32 %15, %34, %52;\n\t"
+      "addc.cc.u32 %16, %35, %53;\n\t"
+      "addc.cc.u32 %17, %36, %54;\n\t"
+      "addc.u32 %18, %55, 0;"
+      : "=r"(z[1]), "=r"(z[2]), "=r"(z[3]), "=r"(z[4]), "=r"(z[5]), "=r"(z[6]), "=r"(z[7]), "=r"(z[8]), "=r"(z[9]), "=r"(z[10]), "=r"(z[11]), "=r"(z[12]), "=r"(z[13]), "=r"(z[14]), "=r"(z[15]), "=r"(z[16]), "=r"(z[17]), "=r"(z[18]), "=r"(z[19])
+      : "r"(el[1]), "r"(el[2]), "r"(el[3]), "r"(el[4]), "r"(el[5]), "r"(el[6]), "r"(el[7]), "r"(el[8]), "r"(el[9]), "r"(el[10]), "r"(el[11]), "r"(el[12]), "r"(el[13]), "r"(el[14]), "r"(el[15]), "r"(el[16]), "r"(el[17]), "r"(el[18]), "r"(ol[0]), "r"(ol[1]), "r"(ol[2]), "r"(ol[3]), "r"(ol[4]), "r"(ol[5]), "r"(ol[6]), "r"(ol[7]), "r"(ol[8]), "r"(ol[9]), "r"(ol[10]), "r"(ol[11]), "r"(ol[12]), "r"(ol[13]), "r"(ol[14]), "r"(ol[15]), "r"(ol[16]), "r"(ol[17]), "r"(ol[18]));
+}
+
 // mod_m and to_ranlux as the hot paths run them: the overwhelmingly likely case, a `rare` flag otherwise;
 // the caller then recomputes with the exact functions above (mod_m20, to_ranlux_exact).
 // Fast fold of z (20 limbs, hi = z[18] + z[19] 2^32 < 2^37) to x = z mod 2^576 - hi + hi 2^240.
@@ -451,7 +488,16 @@ __device__ __forceinline__ void to_ranlux_fast(const u32 (&x)[18], u32 (&v)[18],
 
 }  // namespace detail
 
-class Stream {
+// The multiplier rows of a luxury level baked into the instruction stream: defined by include/rlxpp_rows.cuh for
+// P in {24, 389, 1024, 2048} (include it after this header to use StreamT<P> with P != 0).
+template <int P>
+struct FixedMultiplier;
+
+// P = 0 (rlxpp_dev::Stream): the multiplier a^p is read from the view at run time, any luxury level: the paper's
+// multiply9x9 + mod_m.  P != 0: the luxury level is fixed at compile time and MUST be the handle's; the 324 products
+// take the pre-reduced rows of include/rlxpp_rows.cuh as immediates and mod_m shrinks to a 37-bit fold.
+template <int P = 0>
+class StreamT {
  public:
   // Stream i of the handle behind `view`.
   __device__ __forceinline__ void load(const rlxpp_view_t& view, uint64_t i) {
@@ -463,8 +509,10 @@ class Stream {
     const uint4 q = __ldcg(view.st + 4 * view.n + i);
     x_[16] = q.x; x_[17] = q.y;
     pos_ = q.z > 12u ? 12u : q.z;
+    if (P == 0) {
 #pragma unroll
-    for (int j = 0; j < 18; j++) a_[j] = __ldg(view.A + j);
+      for (int j = 0; j < 18; j++) a_[j] = __ldg(view.A + j);
+    }
     spare_ = 0;
     if (pos_ < 12u) {  // draws left in the current block: rebuild it from the state
       uint32_t c;
@@ -525,10 +573,22 @@ class Stream {
  private:
   // x <- A x mod m, v <- the 24 RANLUX numbers of the new state
   __device__ __forceinline__ void advance(uint32_t (&x)[18], uint32_t (&v)[18]) const {
-    uint32_t r[18], c;
-    detail::mulmod_generic(x, a_, r);
+    uint32_t c;
+    if constexpr (P != 0) {
+      uint64_t E[9], O[9];
+      uint32_t e9, o9, z[20], r[18], rf = 0;
+      FixedMultiplier<P>::mul(x, E, e9, O, o9);
+      detail::merge_eo(E, e9, O, o9, z);
+      detail::fold_fast(z, r, rf);
+      if (__builtin_expect(rf != 0, 0)) detail::mod_m20(z, r);
 #pragma unroll
-    for (int j = 0; j < 18; j++) x[j] = r[j];
+      for (int j = 0; j < 18; j++) x[j] = r[j];
+    } else {
+      uint32_t r[18];
+      detail::mulmod_generic(x, a_, r);
+#pragma unroll
+      for (int j = 0; j < 18; j++) x[j] = r[j];
+    }
     uint32_t rare = 0;
     detail::to_ranlux_fast(x, v, c, rare);  // decides the carry from two leading words; exact form otherwise (~2^-16)
     if (__builtin_expect(rare != 0, 0)) detail::to_ranlux_exact(x, v, c);
@@ -547,10 +607,11 @@ class Stream {
   uint32_t v_[18];   // current block: packed RANLUX numbers
   uint32_t xs_[18];  // spare block (draw_coop): its state ...
   uint32_t vs_[18];  // ... and its numbers
-  uint32_t a_[18];   // a^p
+  uint32_t a_[18];   // a^p (P = 0 only)
   uint32_t pos_;     // draws already taken from the current block, 0..12
   uint32_t spare_;
 };
+typedef StreamT<0> Stream;
 
 }  // namespace rlxpp_dev
 #endif  // RLXPP_DEVICE_CUH

@@ -31,44 +31,7 @@ using rlxpp_dev::detail::mulmod_generic;
 using rlxpp_dev::detail::to_ranlux_exact;
 using rlxpp_dev::detail::fold_fast;
 using rlxpp_dev::detail::to_ranlux_fast;
-
-// ------------------------------------------------------------------ hot-path fast forms
-// Row-reduced product: Z = sum_i x_i R_i < 2^613 arrives as E/O accumulators (see
-// rows_generated.cuh).  merge_eo adds the two interleaved sets into 20 limbs.
-__device__ __forceinline__ void merge_eo(const u64 (&E)[9], u32 e9, const u64 (&O)[9], u32 o9, u32 (&z)[20]) {
-  u32 el[19], ol[19];
-#pragma unroll
-  for (int w = 0; w < 9; w++) {
-    el[2 * w] = (u32)E[w];
-    el[2 * w + 1] = (u32)(E[w] >> 32);
-    ol[2 * w] = (u32)O[w];
-    ol[2 * w + 1] = (u32)(O[w] >> 32);
-  }
-  el[18] = e9;
-  ol[18] = o9;
-  z[0] = el[0];
-  asm("add.cc.u32 %0, %19, %37;\n\t"
-      "addc.cc.u32 %1, %20, %38;\n\t"
-      "addc.cc.u32 %2, %21, %39;\n\t"
-      "addc.cc.u32 %3, %22, %40;\n\t"
-      "addc.cc.u32 %4, %23, %41;\n\t"
-      "addc.cc.u32 %5, %24, %42;\n\t"
-      "addc.cc.u32 %6, %25, %43;\n\t"
-      "addc.cc.u32 %7, %26, %44;\n\t"
-      "addc.cc.u32 %8, %27, %45;\n\t"
-      "addc.cc.u32 %9, %28, %46;\n\t"
-      "addc.cc.u32 %10, %29, %47;\n\t"
-      "addc.cc.u32 %11, %30, %48;\n\t"
-      "addc.cc.u32 %12, %31, %49;\n\t"
-      "addc.cc.u32 %13, %32, %50;\n\t"
-      "addc.cc.u32 %14, %33, %51;\n\t"
-      "addc.cc.u32 %15, %34, %52;\n\t"
-      "addc.cc.u32 %16, %35, %53;\n\t"
-      "addc.cc.u32 %17, %36, %54;\n\t"
-      "addc.u32 %18, %55, 0;"
-      : "=r"(z[1]), "=r"(z[2]), "=r"(z[3]), "=r"(z[4]), "=r"(z[5]), "=r"(z[6]), "=r"(z[7]), "=r"(z[8]), "=r"(z[9]), "=r"(z[10]), "=r"(z[11]), "=r"(z[12]), "=r"(z[13]), "=r"(z[14]), "=r"(z[15]), "=r"(z[16]), "=r"(z[17]), "=r"(z[18]), "=r"(z[19])
-      : "r"(el[1]), "r"(el[2]), "r"(el[3]), "r"(el[4]), "r"(el[5]), "r"(el[6]), "r"(el[7]), "r"(el[8]), "r"(el[9]), "r"(el[10]), "r"(el[11]), "r"(el[12]), "r"(el[13]), "r"(el[14]), "r"(el[15]), "r"(el[16]), "r"(el[17]), "r"(el[18]), "r"(ol[0]), "r"(ol[1]), "r"(ol[2]), "r"(ol[3]), "r"(ol[4]), "r"(ol[5]), "r"(ol[6]), "r"(ol[7]), "r"(ol[8]), "r"(ol[9]), "r"(ol[10]), "r"(ol[11]), "r"(ol[12]), "r"(ol[13]), "r"(ol[14]), "r"(ol[15]), "r"(ol[16]), "r"(ol[17]), "r"(ol[18]));
-}
+using rlxpp_dev::detail::merge_eo;
 
 // ------------------------------------------------------------------ rare-path counters
 // Which condition sent an advance of the hot kernels to the exact code (rlxpp_rare_counts, include/rlxpp.h).  The

@@ -137,13 +137,14 @@ __global__ void __launch_bounds__(kThreads) import_ranlux_kernel(uint4* __restri
 // COOP = draw_coop() (one advance pass per warp and 12 draws whatever the cursors), else draw()
 // (the paper's per-thread advance, which diverges); COOP = 2 alternates the two from draw to draw on the same Stream
 // (they mix freely: a spare block made by draw_coop() is entered by draw()).
-template <int COOP, bool REDUCE>
+// P = the handle's luxury level when it is one of the baked ones (rlxpp_dev::StreamT<P>: rows as immediates), else 0.
+template <int COOP, bool REDUCE, int P = 0>
 __global__ void __launch_bounds__(kThreads) ragged_kernel(const rlxpp_view_t view, const u32* __restrict__ counts,
                                                           double* __restrict__ out, u64 ld, double* __restrict__ sum,
                                                           double* __restrict__ sumsq) {
   const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
   const bool live = i < view.n;
-  rlxpp_dev::Stream g;
+  rlxpp_dev::StreamT<P> g;
   if (live) g.load(view, i);
   const u32 cnt = live ? counts[i] : 0u;
   double S = 0.0, Q = 0.0;

@@ -7,7 +7,7 @@
 //                   matrix of A 2^(8k) mod m, then a 72-column carry normalisation and a 15-bit fold
 //                   (include/rlxpp_tile.cuh, umma_path.cuh, kernels_umma.cuh);
 //                   IMAD engine: 324 IMAD.WIDE.U32.X with the multiplier as immediates, rows pre-reduced mod m
-//                   (rows_generated.cuh, state.cuh, kernels_imad.cuh)
+//                   (include/rlxpp_rows.cuh, state.cuh, kernels_imad.cuh)
 //   to_ranlux    -> 8-limb add + carry decision (to_ranlux_fast; exact fallback)
 //   12 doubles   -> byte permutes + one exact DADD each (emit.cuh); coalesced 64-bit stores (interleaved layout), TMA
 //                   boxes staged in shared memory (stream-major: stages.cuh) or DADD / DFMA accumulation in registers
@@ -28,7 +28,6 @@
 #include "arith.cuh"
 #include "normal_coeffs.cuh"
 #include "host_bigint.h"
-#include "rows_generated.cuh"
 
 namespace rlx {
 
@@ -573,7 +572,7 @@ int rlxpp_create(rlxpp_t** hout, uint64_t n_streams, uint64_t seed, uint32_t p, 
   h->fixed = fixed_level(p, h->tables.A);
   if (h->fixed < 0) {
     delete h;
-    return fail(RLXPP_EINVAL, "rlxpp_create: rows_generated.cuh is stale for p = %u (rebuild)", p);
+    return fail(RLXPP_EINVAL, "rlxpp_create: include/rlxpp_rows.cuh is stale for p = %u (rebuild)", p);
   }
   rc = get_bmatrix(p, &h->bmat);
   if (rc) {
@@ -662,7 +661,7 @@ int rlxpp_advance_states(uint64_t* states_dev, uint64_t n_states, uint32_t p, ui
   if (rc) return rc;
   const Tables& t = cached_tables(p);
   const int fixed = fixed_level(p, t.A);
-  if (fixed < 0) return fail(RLXPP_EINVAL, "rlxpp_advance_states: rows_generated.cuh is stale for p = %u", p);
+  if (fixed < 0) return fail(RLXPP_EINVAL, "rlxpp_advance_states: include/rlxpp_rows.cuh is stale for p = %u", p);
   cudaStream_t s = (cudaStream_t)cuda_stream;
   if (g_engine.load() == RLXPP_ENGINE_UMMA) {
     const uint4* bmat = nullptr;
@@ -1018,15 +1017,27 @@ static int launch_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out, ui
     LAUNCH_CHECK();
     return RLXPP_OK;
   }
-  if (reduce) {
-    if (coop == 2) ragged_kernel<2, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-    else if (coop) ragged_kernel<1, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-    else ragged_kernel<0, true><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-  } else {
-    if (coop == 2) ragged_kernel<2, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-    else if (coop) ragged_kernel<1, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
-    else ragged_kernel<0, false><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq);
+  // the per-thread generator with the handle's luxury level baked in when it is one of the generated ones
+#define RLXPP_RAGGED(COOP, RED, P) ragged_kernel<COOP, RED, P><<<grid, kThreads, 0, h->stream>>>(view, counts_dev, out, ld, sum, sumsq)
+#define RLXPP_CASE(P)                                      \
+  if (h->fixed == P && coop != 2) {                        \
+    if (reduce) { if (coop) RLXPP_RAGGED(1, true, P); else RLXPP_RAGGED(0, true, P); }   \
+    else { if (coop) RLXPP_RAGGED(1, false, P); else RLXPP_RAGGED(0, false, P); }        \
+    LAUNCH_CHECK();                                        \
+    return RLXPP_OK;                                       \
   }
+  RLXPP_FOR_EACH_FIXED_P(RLXPP_CASE)
+#undef RLXPP_CASE
+  if (reduce) {
+    if (coop == 2) RLXPP_RAGGED(2, true, 0);
+    else if (coop) RLXPP_RAGGED(1, true, 0);
+    else RLXPP_RAGGED(0, true, 0);
+  } else {
+    if (coop == 2) RLXPP_RAGGED(2, false, 0);
+    else if (coop) RLXPP_RAGGED(1, false, 0);
+    else RLXPP_RAGGED(0, false, 0);
+  }
+#undef RLXPP_RAGGED
   LAUNCH_CHECK();
   return RLXPP_OK;
 }

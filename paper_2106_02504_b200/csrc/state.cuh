@@ -3,10 +3,11 @@
 #pragma once
 
 #include "arith.cuh"
-#include "rows_generated.cuh"
+#include "../../include/rlxpp_rows.cuh"
 
 namespace rlx {
 
+using rlxpp_dev::FixedMultiplier;
 constexpr int kThreads = 128;  // threads per CTA of the one-thread-per-stream kernels = streams per UMMA tile
 
 // ----------------------------------------------------------------------------- state I/O

@@ -461,8 +461,9 @@ def test_p24_floats_are_the_raw_ranlux_numbers(rlx, torch, oracle):
 
 
 # ------------------------------------------------------------------------------------- device API (8f-1)
+@pytest.mark.parametrize("p", [2048, 100])
 @pytest.mark.parametrize("coop", [True, False, 2, 3])
-def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, coop):
+def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, coop, p):
     """include/rlxpp_device.cuh through rlxpp_generate_ragged: every stream draws its own number of
     doubles (0 .. 70, so lanes of a warp run out of their blocks at different calls), from per-stream
     cursors, twice in a row, then the library's bulk kernel continues the same streams.  Everything
@@ -470,8 +471,9 @@ def test_device_api_ragged_draws_match_the_stream(rlx, torch, oracle, nthreads, 
     and so does a kernel that alternates draw_coop() and draw() on the same Stream (coop = 2: a spare block
     made by draw_coop() must be entered, not recomputed past, by draw()); coop = 3 is include/rlxpp_tile.cuh's
     rlxpp_dev::TileStream, the block-cooperative tensor-core advance (ragged counts: threads ask for passes at different
-    calls, some threads of a CTA are done long before others, the last CTA is ragged)."""
-    n, p, ld = 1000, 2048, 72
+    calls, some threads of a CTA are done long before others, the last CTA is ragged).  p = 2048 takes the per-thread
+    generator with the rows baked in (rlxpp_dev::StreamT<2048>, include/rlxpp_rows.cuh), p = 100 the run-time multiplier."""
+    n, ld = 1000, 72
     dist = inputs.splitmix64(77, n) % np.uint64(30)
     c1 = (inputs.splitmix64(78, n) % np.uint64(71)).astype(np.uint32)
     c2 = (inputs.splitmix64(79, n) % np.uint64(71)).astype(np.uint32)

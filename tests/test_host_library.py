@@ -123,7 +123,7 @@ def test_host_engine_matches_big_integer_model(p):
         rlx.rlxpp_host_generate(_limbs(1), 13, p, 0, 1)
 
 
-@pytest.mark.parametrize("example", ["device_api_example.cu", "tile_api_example.cu"])
+@pytest.mark.parametrize("example", ["device_api_example.cu", "tile_api_example.cu", "fixed_api_example.cu"])
 def test_public_device_header_is_self_contained(tmp_path, example):
     """include/rlxpp_device.cuh (per-thread generator) and include/rlxpp_tile.cuh (block-cooperative tensor-core
     advance) alone are enough to write a kernel: nvcc compiles a user kernel that includes nothing else
@@ -140,7 +140,7 @@ def test_public_device_header_is_self_contained(tmp_path, example):
 
 
 def test_fixed_multiplier_rows_header_is_what_its_generator_writes(tmp_path):
-    """csrc/rows_generated.cuh (the IMAD engine's 4 x 324 immediates) is committed although build() regenerates it;
+    """include/rlxpp_rows.cuh (the IMAD engine's 4 x 324 immediates) is committed although build() regenerates it;
     it must be exactly csrc/gen_rows.py's output, and its immediates must be the limbs of A 2^(32 i) mod m."""
     import importlib.util
     import re
@@ -148,9 +148,9 @@ def test_fixed_multiplier_rows_header_is_what_its_generator_writes(tmp_path):
     spec = importlib.util.spec_from_file_location("gen_rows", os.path.join(here, "gen_rows.py"))
     gen = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(gen)
-    tracked = open(os.path.join(here, "rows_generated.cuh")).read()
+    tracked = open(os.path.join(ROOT, "include", "rlxpp_rows.cuh")).read()
     body = "\n\n".join(gen.emit_level(p) for p in gen.LEVELS)
-    assert body in tracked, "rows_generated.cuh is stale: run python -m paper_2106_02504_b200.build"
+    assert body in tracked, "include/rlxpp_rows.cuh is stale: run python -m paper_2106_02504_b200.build"
     # the immediates themselves, against Python: row i of level p = limbs of a^p 2^(32 i) mod m (324 per level)
     for p, block in zip(gen.LEVELS, re.split(r"// ---- p = \d+:", tracked)[1:]):
         A = pow(A1, p, M)
