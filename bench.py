@@ -471,6 +471,24 @@ def main():
                                   "ncu --set full capture of this kernel (another run of the same build), not this run")
     roofline["per_launch_ms"] = launch_spread
 
+    # ---------------------------------------------------------------- the other engine, same workload (context; before the
+    # sustained leg, which leaves the chip at its power-capped clocks)
+    compare = None
+    if not args.no_compare and args.workload != "devapi" and args.output == "f64":
+        other = "imad" if umma else "umma"
+        rlx.rlxpp_set_engine(engines[other])
+        step()
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
+        for _ in range(3):
+            step()
+        c1.record(stream)
+        torch.cuda.synchronize()
+        compare = {"engine": other, "value": units / (c0.elapsed_time(c1) / 3 * 1e-3), "unit": UNIT, "steps": 3,
+                   "n_gpus": 1, "what": "same workload and launch configuration with the other engine, this rank only"}
+        rlx.rlxpp_set_engine(engines[args.engine])
+
     # ---------------------------------------------------------------- sustained: the same step for >= 3 s
     sustained = None
     if args.sustained_s > 0 and rank == 0:
@@ -498,23 +516,6 @@ def main():
                      "roofline_frac": roofline["frac"] * kernel_ms / s_ms, "clocks": s_clocks,
                      "what": f"the timed step repeated back to back for >= {args.sustained_s:g} s on this rank, CUDA events every "
                              f"{block} launches; NVML clocks / power / reasons sampled throughout"}
-
-    # ---------------------------------------------------------------- the other engine, same workload (context)
-    compare = None
-    if not args.no_compare and args.workload != "devapi" and args.output == "f64":
-        other = "imad" if umma else "umma"
-        rlx.rlxpp_set_engine(engines[other])
-        step()
-        torch.cuda.synchronize()
-        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        c0.record(stream)
-        for _ in range(3):
-            step()
-        c1.record(stream)
-        torch.cuda.synchronize()
-        compare = {"engine": other, "value": units / (c0.elapsed_time(c1) / 3 * 1e-3), "unit": UNIT, "steps": 3,
-                   "n_gpus": 1, "what": "same workload and launch configuration with the other engine, this rank only"}
-        rlx.rlxpp_set_engine(engines[args.engine])
 
     devapi = None
     if args.workload == "devapi":
