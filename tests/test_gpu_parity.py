@@ -649,7 +649,7 @@ def test_chunked_work_items_give_the_same_results(rlx, torch, oracle, nthreads, 
 @pytest.mark.parametrize("blocks", [1, 7, 8, 9, 15, 16, 21, 43])
 def test_stream_major_rows_of_any_length(rlx, torch, oracle, nthreads, blocks):
     """Stream-major output, aligned cursors (UMMA engine: 256-byte boxes through the TMA for whole cycles of
-    8 blocks, direct stores for the rest of a row; rlxpp.cu StreamMajorStage).  Row lengths on both sides of
+    8 blocks, direct stores for the rest of a row; csrc/stages.cuh StreamMajorStage).  Row lengths on both sides of
     the cycle, rows that are not 128- or 256-byte multiples, a ragged last warp and tile (rows the tensor
     map must clip), and a guard band behind the buffer that must stay untouched.  Two calls in a row: the
     second continues the streams."""
@@ -923,7 +923,7 @@ def test_errors_of_the_widened_calls_and_the_store_probe(rlx, torch):
 @pytest.mark.parametrize("n", [3 * 128 + 44, 3 * 128 + 45])
 def test_interleaved_floats_through_row_boxes(rlx, torch, oracle, nthreads, blocks, n):
     """rlxpp_generate_floats, interleaved, aligned cursors (UMMA engine: the CTA's block leaves as one TMA box of
-    24 float rows x 128 streams, three boxes in flight; rlxpp.cu F32RowStage).  1, 2, 3 blocks (fewer than the ring),
+    24 float rows x 128 streams, three boxes in flight; csrc/stages.cuh F32RowStage).  1, 2, 3 blocks (fewer than the ring),
     more; a ragged last tile the tensor map must clip; n not a multiple of 4 takes the direct stores; forced chunks;
     the guard band stays untouched; two calls in a row."""
     per = 12 * blocks
@@ -996,7 +996,7 @@ def test_eight_shard_handles_reproduce_one_generator(rlx, torch, oracle, nthread
 @pytest.mark.parametrize("n, blocks", [(1024, 32), (128 * 20 + 77, 32), (128 * 60, 40), (5, 4), (128 * 140 + 3, 7), (700, 100)])
 def test_short_calls_run_time_parallel(rlx, torch, oracle, nthreads, n, blocks):
     """UMMA engine, calls that leave most of the grid empty (cfg1's shape): K lanes per tile, lane j reaching block j with
-    the byte matrix of A^(j+1) and striding with the one of A^K (rlxpp.cu tc_generate_lanes_kernel; reading D7: block b is
+    the byte matrix of A^(j+1) and striding with the one of A^K (csrc/kernels_umma.cuh tc_generate_lanes_kernel; reading D7: block b is
     to_ranlux(A^(b+1) X)).  One pass per lane (32 blocks, K = 32), several passes (K = 9 / 29 / 4: 60 or 21 tiles; 100 blocks),
     a 5-stream handle, a grid that is too full for lanes (141 tiles: the persistent path), ragged tiles; every output form
     and layout; the state each call leaves is the one the next call starts from; guard bands stay untouched."""
@@ -1040,7 +1040,7 @@ def test_short_calls_run_time_parallel(rlx, torch, oracle, nthreads, n, blocks):
 def test_stream_major_per_stream_cursors_through_rings(rlx, torch, oracle, nthreads, per, n_chunks):
     """Stream-major output when the cursors are not at a block boundary (per-stream skips; one odd common cursor).  UMMA
     engine, even row length: every lane writes its 12 doubles at its own columns of a shared-memory ring and the warp sends
-    128-byte granules of 32 rows as TMA boxes once its slowest lane has completed them (rlxpp.cu RingStage); row ends and
+    128-byte granules of 32 rows as TMA boxes once its slowest lane has completed them (csrc/stages.cuh RingStage); row ends and
     rows past the launch are clipped by the tensor map.  Rows of 2 doubles up to cfg3's 1,536, a length that is not a
     multiple of 16, forced chunks (granule-aligned item starts), a ragged last tile, all 8-byte output forms, the guard
     band behind the buffer, two calls in a row; per = 251 (odd pitch) takes the element-wise row stage instead."""
