@@ -84,6 +84,43 @@ __device__ __forceinline__ void mma_i8(u32 d_tmem, u64 adesc, u64 bdesc, u32 ide
       : "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+// The same with A read from tensor memory (lane = row, 8 columns of 32 bits = the 32 K bytes of one MMA).
+__device__ __forceinline__ void mma_i8_ts(u32 d_tmem, u32 a_tmem, u64 bdesc, u32 idesc, u32 accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t"
+      "}"
+      :
+      : "r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// tcgen05.st 32x32b: thread t of warp w writes N consecutive 32-bit columns of TMEM lane 32 (w % 4) + t.
+__device__ __forceinline__ void tmem_st18(u32 taddr, const u32 (&x)[18]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17};\n\t"
+      "tcgen05.st.sync.aligned.32x32b.x2.b32 [%1], {%18, %19};"
+      :
+      : "r"(taddr), "r"(taddr + 16u), "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(x[7]),
+        "r"(x[8]), "r"(x[9]), "r"(x[10]), "r"(x[11]), "r"(x[12]), "r"(x[13]), "r"(x[14]), "r"(x[15]), "r"(x[16]), "r"(x[17])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_zero8(u32 taddr) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %1, %1, %1, %1, %1, %1, %1};" ::"r"(taddr), "r"(0u) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// ... and back: 18 columns, then tcgen05.wait::ld
+__device__ __forceinline__ void tmem_ld18_wait(u32 taddr, u32 (&x)[18]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%18];\n\t"
+      "tcgen05.ld.sync.aligned.32x32b.x2.b32 {%16, %17}, [%19];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=r"(x[0]), "=r"(x[1]), "=r"(x[2]), "=r"(x[3]), "=r"(x[4]), "=r"(x[5]), "=r"(x[6]), "=r"(x[7]), "=r"(x[8]), "=r"(x[9]),
+        "=r"(x[10]), "=r"(x[11]), "=r"(x[12]), "=r"(x[13]), "=r"(x[14]), "=r"(x[15]), "=r"(x[16]), "=r"(x[17])
+      : "r"(taddr), "r"(taddr + 16u)
+      : "memory");
+}
 // arrive on the mbarrier once every tcgen05.mma issued so far by this thread has completed
 // (implies tcgen05.fence::before_thread_sync)
 __device__ __forceinline__ void commit(u32 bar) {

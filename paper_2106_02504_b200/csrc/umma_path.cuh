@@ -18,15 +18,19 @@
 // fma-heavy pipe) by ~75 plain integer instructions.
 //
 // Protocol per CTA (128 threads = 128 streams = UMMA M = the 128 TMEM lanes), per advance:
-//   issue():   every thread stores its 72 state bytes into the K-major A tile in shared memory
-//              (generic proxy) -> fence.proxy.async -> tcgen05.fence::before_thread_sync ->
-//              __syncthreads -> thread 0: tcgen05.fence::after_thread_sync, 3 x tcgen05.mma,
-//              tcgen05.commit -> mbarrier
+//   issue():   every thread stores its 72 state bytes as 18 columns of its own TENSOR-MEMORY lane (tcgen05.st: the A
+//              operand is read from tensor memory, lane = row, 8 columns = the 32 K bytes of one MMA) ->
+//              tcgen05.wait::st -> tcgen05.fence::before_thread_sync -> hand-off barrier -> one thread:
+//              tcgen05.fence::after_thread_sync, 3 x tcgen05.mma, tcgen05.commit -> mbarrier
 //   (the threads convert and emit the PREVIOUS block's doubles while the tensor core works)
 //   collect(): mbarrier wait -> tcgen05.fence::after_thread_sync -> tcgen05.ld of 72 columns ->
 //              tcgen05.wait::ld -> normalise.
 // The next issue() orders the TMEM reads before the next MMA's TMEM writes (fence + barrier),
-// and the mbarrier wait orders the MMA's shared-memory reads before the next A-tile stores.
+// and the mbarrier wait orders the MMA's reads of the A columns before the next tcgen05.st to them.
+// (Round 1 and most of round 2 kept the A tile in shared memory: five st.shared.v4 and a fence.proxy.async -- SASS
+// MEMBAR.ALL.CTA + FENCE.VIEW.ASYNC -- per advance and thread, and 12 KB of operand reads per MMA.  An allocation of
+// 128 columns holds the accumulator (80) AND two operands (24 each); same results, less energy:
+// profiles/ab_r02_pairs.md section 6.  GroupTile below still uses shared memory: six accumulators leave no columns.)
 #pragma once
 #include "arith.cuh"
 #include "umma.cuh"
@@ -49,8 +53,12 @@ using rlxpp_dev::tile::normalise;
 // K columns of the byte matrix that are filled: the 72 bytes of a state, and bytes 72, 73 for operands that are products
 // not yet folded (Z < 2^591: the raw advance keeps its state unreduced between repetitions, GroupTile::stash19)
 constexpr int kKUsed = 74;
+// A operands in tensor memory: operand t of an allocation at columns kACol + t kACols .. (96 K bytes = 24 columns)
+constexpr u32 kACol = (u32)kN;
+constexpr u32 kACols = 24;
+static_assert(kACol + 2 * kACols <= kTmemCols, "accumulator + two A operands in one allocation");
 
-// How the CTA hands the freshly written A tile to the thread that issues the MMAs.
+// How the CTA hands the freshly written A operand to the thread that issues the MMAs.
 //   kSyncCta:    __syncthreads, warp 0 issues.  Every warp waits for the slowest one.
 //   kSyncArrive: named barrier 1 -- three warps `bar.arrive` and go straight on to their doubles, only the
 //                issuing warp `bar.sync`s (asleep, no polling).  The issuing warp is rotated over the
@@ -61,7 +69,6 @@ constexpr int kKUsed = 74;
 enum { kSyncCta = 0, kSyncArrive = 2 };
 
 struct Smem {
-  __align__(128) uint8_t a[kABytes];
   __align__(128) uint8_t b[kBBytes];
   __align__(8) u64 bar;        // MMA done (tcgen05.commit)
   u32 tmem_slot;
@@ -70,22 +77,18 @@ struct Smem {
 
 template <int SYNC>
 struct Tile {
-  u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of the A tile
   u32 bar;
   u32 phase;
   u32 tmem;    // TMEM base address of the accumulator (lane 0, first column)
   u32 tld;     // the same with this warp's lane quarter in bits [16,32)
   u32 issuer;         // the warp that issues this CTA's MMAs
-  u64 adesc, bdesc;
+  u64 bdesc;
 
   // CTA-collective.  bmat: device pointer to the kBBytes image of B.
   __device__ __forceinline__ void setup(Smem& s, const uint4* __restrict__ bmat) {
     const u32 tid = threadIdx.x;
     uint4* sb = reinterpret_cast<uint4*>(s.b);
     for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
-    a_row = umma::smem_u32(s.a) + tid * 16u;
-    // K bytes 80..95 of every row stay zero for the whole kernel
-    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a_row + 5u * kAChunk), "r"(0u) : "memory");
     bar = umma::smem_u32(&s.bar);
     phase = 0;
     if (tid == 0) {
@@ -102,7 +105,7 @@ struct Tile {
     tmem = *reinterpret_cast<volatile u32*>(&s.tmem_slot);
     issuer = SYNC == kSyncArrive ? ((tmem & 0xFFFFu) / kTmemCols) & 3u : 0u;
     tld = tmem + (((tid >> 5) & 3u) << 21);  // lane 32 (warp % 4) in bits [16,32)
-    adesc = umma::smem_desc(umma::smem_u32(s.a), kAChunk, 128u);
+    umma::tmem_st_zero8(tld + kACol + 16u);  // K bytes 72..95 of every row stay zero (issue() rewrites columns 16, 17)
     bdesc = umma::smem_desc(umma::smem_u32(s.b), kBChunk, 128u);
   }
 
@@ -115,14 +118,8 @@ struct Tile {
   // async-proxy work on the CTA's shared memory that must be ordered with the MMA-done mbarrier (F32RowStage).
   template <class Before, class After>
   __device__ __forceinline__ void issue(const u32 (&x)[18], Before&& before, After&& after) {
-#pragma unroll
-    for (int g = 0; g < 4; g++)
-      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a_row + (u32)g * kAChunk), "r"(x[4 * g]),
-                   "r"(x[4 * g + 1]), "r"(x[4 * g + 2]), "r"(x[4 * g + 3])
-                   : "memory");
-    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(a_row + 4u * kAChunk), "r"(x[16]), "r"(x[17]), "r"(0u)
-                 : "memory");
-    umma::fence_proxy_async_smem();
+    umma::tmem_st18(tld + kACol, x);
+    umma::tmem_wait_st();
     umma::fence_before_sync();
     if (SYNC == kSyncArrive) {
       if ((threadIdx.x >> 5) == issuer) {
@@ -141,12 +138,12 @@ struct Tile {
     }
   }
 
-  // One thread: D = Xbytes * B^T as three K steps of 32 bytes (two 16-byte chunks each).
+  // One thread: D = Xbytes * B^T as three K steps of 32 bytes (A: 8 columns each; B: two 16-byte chunks each).
   __device__ __forceinline__ void issue_mma() {
     umma::fence_after_sync();
 #pragma unroll
     for (u32 k = 0; k < 3; k++)
-      umma::mma_i8(tmem, adesc + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
+      umma::mma_i8_ts(tmem, tmem + kACol + 8u * k, bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
     umma::commit(bar);
   }
 
@@ -171,24 +168,23 @@ struct Tile {
 
 // ---------------------------------------------------------------------------------------------------------------
 // Two tiles per CTA on ONE accumulator (the kernels no store path binds: fused reduce, raw advance).
-// A tile's advances are a serial chain  MMA -> tcgen05.ld -> normalise + fold -> A-tile store -> MMA ..., and with one
+// A tile's advances are a serial chain  MMA -> tcgen05.ld -> normalise + fold -> A-operand store -> MMA ..., and with one
 // tile per CTA the threads sit idle for the MMA + commit + mbarrier round trip of every advance; TMEM (4 x 128
 // allocated columns) caps the SM at four such chains.  The accumulator, however, is only live between the MMA and
 // the tcgen05.ld that empties it into registers.  So a CTA of 128 threads owns TWO tiles (thread r = stream r of
-// both), each with its own A tile in shared memory, sharing the 80 accumulator columns in time:
+// both), each with its own A operand in tensor memory, sharing the 80 accumulator columns in time:
 //
 //     load(t):   wait for MMA(t)  ->  tcgen05.ld + wait::ld                  (accumulator now free)
-//     start(t'): hand-off barrier ->  issuing thread: MMA(t') + commit       (t' = the other tile; its A tile was
+//     start(t'): hand-off barrier ->  issuing thread: MMA(t') + commit       (t' = the other tile; its A operand was
 //                                                                             stored in the previous half-step)
 //     normalise + fold tile t, stash(t) its new state for the next MMA(t), convert and consume its block
 //
 // MMA(t') runs under the ~250 instructions per warp of tile t's integer work: 8 chains per SM with the same 16 warps,
 // same TMEM, and no thread ever waits for the tensor pipe's round trip.  Ordering: every thread's tcgen05.ld of
 // the accumulator is complete (wait::ld, fence::before_thread_sync) before the hand-off barrier that precedes the next
-// MMA; MMA(t)'s reads of A tile t are complete (mbarrier) before stash(t) overwrites it; one mbarrier serves both
+// MMA; MMA(t)'s reads of A operand t are complete (mbarrier) before stash(t) overwrites it; one mbarrier serves both
 // tiles because at most one commit is ever outstanding.
 struct PairSmem {
-  __align__(128) uint8_t a[2][kABytes];
   __align__(128) uint8_t b[kBBytes];
   __align__(8) u64 bar;
   u32 tmem_slot;
@@ -197,9 +193,8 @@ struct PairSmem {
 
 template <int SYNC>
 struct PairTile {
-  u32 a_row;   // shared address of this thread's 16-byte row slot in K chunk 0 of A tile 0 (tile 1: + kABytes)
   u32 bar, phase, tmem, tld, issuer;
-  u64 adesc, bdesc;  // adesc: A tile 0
+  u64 bdesc;
   u32 tid;           // thread within the tile (= stream within each of the two tiles)
   u32* ticket;       // shared word of the persistent scheduler
 
@@ -210,10 +205,6 @@ struct PairTile {
     ticket = &s.ticket;
     uint4* sb = reinterpret_cast<uint4*>(s.b);
     for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
-    a_row = umma::smem_u32(s.a[0]) + tid * 16u;
-#pragma unroll
-    for (u32 t = 0; t < 2; t++)  // K bytes 80..95 of every row stay zero for the whole kernel
-      asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(a_row + t * kABytes + 5u * kAChunk), "r"(0u) : "memory");
     bar = umma::smem_u32(&s.bar);
     phase = 0;
     if (tid == 0) {
@@ -230,24 +221,18 @@ struct PairTile {
     tmem = *reinterpret_cast<volatile u32*>(&s.tmem_slot);
     issuer = SYNC == kSyncArrive ? ((tmem & 0xFFFFu) / kTmemCols) & 3u : 0u;
     tld = tmem + (((tid >> 5) & 3u) << 21);
-    adesc = umma::smem_desc(umma::smem_u32(s.a[0]), kAChunk, 128u);
+#pragma unroll
+    for (u32 t = 0; t < 2; t++)  // K bytes 72..95 of every row stay zero (stash() rewrites columns 16, 17)
+      umma::tmem_st_zero8(tld + kACol + t * kACols + 16u);
     bdesc = umma::smem_desc(umma::smem_u32(s.b), kBChunk, 128u);
   }
 
-  // this thread's state of tile t -> A tile t (any value < 2^576), visible to the tensor core after the next start(t)
-  __device__ __forceinline__ void stash(u32 t, const u32 (&x)[18]) {
-    const u32 row = a_row + t * kABytes;
-#pragma unroll
-    for (int g = 0; g < 4; g++)
-      asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(row + (u32)g * kAChunk), "r"(x[4 * g]), "r"(x[4 * g + 1]),
-                   "r"(x[4 * g + 2]), "r"(x[4 * g + 3])
-                   : "memory");
-    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %3};" ::"r"(row + 4u * kAChunk), "r"(x[16]), "r"(x[17]), "r"(0u) : "memory");
-    umma::fence_proxy_async_smem();
-  }
+  // this thread's state of tile t -> A operand t (any value < 2^576), visible to the tensor core after the next start(t)
+  __device__ __forceinline__ void stash(u32 t, const u32 (&x)[18]) { umma::tmem_st18(tld + kACol + t * kACols, x); }
 
   // CTA-collective: every thread has stashed tile t and emptied the accumulator; D = Xbytes(t) * B^T starts
   __device__ __forceinline__ void start(u32 t) {
+    umma::tmem_wait_st();
     umma::fence_before_sync();
     if (SYNC == kSyncArrive) {
       if ((threadIdx.x >> 5) == issuer) {
@@ -265,10 +250,9 @@ struct PairTile {
   }
   __device__ __forceinline__ void issue_mma(u32 t) {
     umma::fence_after_sync();
-    const u64 ad = adesc + (u64)((t * kABytes) >> 4);
 #pragma unroll
     for (u32 k = 0; k < 3; k++)
-      umma::mma_i8(tmem, ad + (u64)((2u * k * kAChunk) >> 4), bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
+      umma::mma_i8_ts(tmem, tmem + kACol + t * kACols + 8u * k, bdesc + (u64)((2u * k * kBChunk) >> 4), kIdesc, k);
     umma::commit(bar);
   }
 
