@@ -379,11 +379,11 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
   constexpr bool kPairs = MODE == kReduce || (MODE == kStoreInterleaved && OUT != kF32);
   const uint64_t n_tiles = kPairs ? (a.count + 2 * tc::kTile - 1) / (2 * tc::kTile) : (a.count + tc::kTile - 1) / tc::kTile;
   // stream-major rows shifted against each other go through per-lane rings and TMA boxes when the rows are 16-byte
-  // aligned (even pitch; RingStage: 69 KB of shared memory, three CTAs per SM), else through the warp's row stage
+  // aligned (even pitch; RingStage: 57 KB of shared memory, three CTAs per SM), else through the warp's row stage
   const uint64_t row_pitch = a.pitch ? a.pitch : a.n_per;
   const bool ring = MODE == kStoreStreamMajor && !aligned && row_pitch % 2 == 0 && (uintptr_t)a.out % 16 == 0 &&
                     a.count < (1ull << 31) && a.n_per < (1ull << 31);
-  const unsigned slots = ring ? tc_slots() / tc::kCtasPerSm * 3 : tc_slots();
+  const unsigned slots = ring ? tc_slots() / tc::kCtasPerSm * 3 : tc_slots();  // (a fourth CTA per SM fits since the A operands left shared memory: measured, no gain)
   a.n_tiles = (u32)n_tiles;
   if constexpr (MODE != kReduce) {
     // Short calls that leave most of the grid empty: K lanes per tile, each reaching its blocks with the matrices of
@@ -435,7 +435,7 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     else tc_pair_kernel<false, MODE, OUT><<<grid, tc::kTile, 0, s>>>(a);
   } else if (aligned) {
     constexpr bool kStaged = MODE == kStoreStreamMajor;  // the kernel's kStaged
-    // 20 KB static + 33 KB (stream-major boxes) or 36 KB (float-row boxes): above the 48 KB default, 4 CTAs per SM fit
+    // 8 KB static + 33 KB (stream-major boxes) or 36 KB (float-row boxes): the function attribute is needed above 48 KB in all; 4 CTAs per SM fit
     if (kStaged || a.f32_boxes) {
       static std::atomic<uint64_t> done{0};  // one bit per device: function attributes are per device
       const int rc = allow_dynamic_smem(tc_generate_kernel<MODE, true, OUT>, done, (int)(kStaged ? kStageCtaBytes : kF32StageBytes));
@@ -447,7 +447,7 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
     if (ring) {
       int rc = encode_ring_map(&a.tmap, a.out, a.count, a.n_per, row_pitch);
       if (rc) return rc;
-      static std::atomic<uint64_t> done{0};  // 20 KB static + 49 KB of rings: three CTAs per SM
+      static std::atomic<uint64_t> done{0};  // 8 KB static + 49 KB of rings
       rc = allow_dynamic_smem(tc_generate_kernel<MODE, false, OUT>, done, (int)kRingCtaBytes);
       if (rc) return rc;
       a.ring = 1;
