@@ -64,8 +64,10 @@ static_assert(kACol + 2 * kACols <= kTmemCols, "accumulator + two A operands in 
 //                issuing warp `bar.sync`s (asleep, no polling).  The issuing warp is rotated over the
 //                SM's co-resident CTAs (warp w always runs on scheduler w % 4; the TMEM column base
 //                0 / 128 / 256 / 384 is unique per resident CTA), so the four schedulers share the
-//                issue work.  Measured (profiles/ab_r01_sync.md): +14 % on the store kernels, +5 % on
-//                the raw advance, -6 % on the fused reduce, which therefore keeps kSyncCta.
+//                issue work.  Measured (profiles/ab_r01_sync.md): +14 % on the store kernels; on the fused
+//                reduce -6 % in round 1 (A tile in shared memory: the hand-off sat behind a MEMBAR.ALL.CTA
+//                anyway) and +7 % now that the operand is in tensor memory (profiles/ab_r02_pairs.md section 6).
+//                kSyncCta is left for the time-parallel lanes kernel (one pass per CTA and a CTA barrier of its own).
 enum { kSyncCta = 0, kSyncArrive = 2 };
 
 struct Smem {
@@ -404,8 +406,9 @@ struct GroupTile {
   }
   __device__ __forceinline__ void start(u32 t) {
     umma::fence_before_sync();
-    // (all 128 threads bar.sync: the group's barrier also serves the raw state staging, so an arrive-and-run-on
-    // hand-off as in PairTile could count a warp twice in one phase)
+    // (All 128 threads bar.sync.  An arrive-and-run-on hand-off as in PairTile needs a barrier of its own -- on the one
+    // that also serves the raw state staging a warp that ran on arrives twice in one phase: deadlock -- and, with ids
+    // 7 .. 12 and the issuing warps spread over the schedulers, measured the same: 1,467 vs 1,469.)
     sync();
     if (tid < 32) {
       if (umma::elect_one()) {
