@@ -196,11 +196,12 @@ using umma::u64;
 constexpr int kTile = 128;                    // streams per CTA = UMMA M
 constexpr int kN = 80;                        // UMMA N (72 byte columns, padded to a multiple of 16)
 constexpr int kKChunks = 6;                   // 16-byte K chunks: 96 bytes of K = 3 MMAs of K = 32
-constexpr u32 kAChunk = kTile * 16;           // bytes of one K chunk of the A tile (16 row groups x 128 B)
+constexpr u32 kAChunk = kTile * 16;           // bytes of one K chunk of a shared-memory A tile (16 row groups x 128 B):
+                                              // TileStream and the library's group kernel; its other kernels keep A in TMEM
 constexpr u32 kBChunk = kN * 16;              // same for B (10 row groups x 128 B)
 constexpr u32 kABytes = kKChunks * kAChunk;   // 12,288
 constexpr u32 kBBytes = kKChunks * kBChunk;   // 7,680
-constexpr u32 kTmemCols = 128;                // power of two >= kN
+constexpr u32 kTmemCols = 128;                // power of two >= kN (the library: kN + two A operands of 24 columns)
 constexpr int kCtasPerSm = 4;                 // 4 x 128 = the SM's 512 TMEM columns
 constexpr u32 kIdesc = umma::idesc_u8u8_s32(kTile, kN);
 
