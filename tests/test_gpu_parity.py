@@ -7,6 +7,8 @@ Small cases span several 128-thread blocks and a ragged tail and are compared in
 BASELINE.json full sizes run in bench.py's launch configuration and are compared on sampled
 streams (the oracle computes any stream on its own) plus size-independent properties.
 """
+from fractions import Fraction
+
 import numpy as np
 import pytest
 
@@ -1082,4 +1084,56 @@ def test_stream_major_per_stream_cursors_through_rings(rlx, torch, oracle, nthre
     assert_within_ulps(z.cpu().numpy(), want, NORMAL_ULPS, f"normals through rings, rows of {per_n}")
     ref2 = oracle.streams(inputs.seeds(n, 17), 2048, 0, skips=g + np.uint64(per_n), want=("state",), nthreads=nthreads)
     check_state(rlx, torch, h, ref2, "after ring calls")
+    rlx.rlxpp_destroy(h)
+
+
+@pytest.mark.parametrize("form", ["stream_major", "interleaved", "reduce", "lanes"])
+def test_one_hot_state_bytes_reach_their_operand_column(rlx, torch, oracle, form):
+    """The A operand of the tensor-core advance is written per thread into tensor memory (18 columns of 32 bits, four K
+    bytes each; csrc/umma_path.cuh) or, for the raw advance, into a K-major shared-memory tile.  States with ONE non-zero
+    byte -- 2^(8k) and 255 * 2^(8k) for every k < 72 -- pin byte order and column order of that operand: the block each
+    produces is to_ranlux(A * x mod m) (D5, D6), row k of the byte matrix scaled.  Every kernel form that writes the
+    operand: one tile per CTA (stream-major), two tiles per CTA (interleaved, fused reduce), time-parallel lanes."""
+    xs = [v << (8 * k) for k in range(72) for v in (1, 255)] + [M - 1]
+    xs = [x for x in xs if x < M]
+    n = len(xs)
+    states = np.stack([inputs.int_to_limbs(x) for x in xs])
+    h = rlx.rlxpp_create(n, 1, 2048)
+    rlx.rlxpp_set_state(h, torch.from_numpy(states.view(np.int64)).cuda(), None)
+    blocks = 8 if form == "lanes" else 2
+    per = 12 * blocks
+    A = oracle.multiplier(2048)
+    want = np.empty((n, per), dtype=np.uint64)
+    for i, x in enumerate(xs):
+        for b in range(blocks):
+            x = oracle.mulmod(A, x)
+            V, _ = oracle.to_ranlux(x)
+            want[i, 12 * b:12 * b + 12] = [(V >> (48 * j)) & (2**48 - 1) for j in range(12)]
+    if form == "reduce":
+        s = torch.empty(n, dtype=torch.float64, device="cuda")
+        q = torch.empty(n, dtype=torch.float64, device="cuda")
+        rlx.rlxpp_generate_reduce(h, s, q, per)
+        d = want.astype(np.float64) * 2.0**-48
+        S = np.zeros(n)
+        Q = np.zeros(n)
+        for k in range(per):  # draw order, one rounding per step (c-14); d*d + Q in exact arithmetic, rounded once
+            S = S + d[:, k]
+            Q = np.array([float(Fraction(float(a)) * Fraction(float(a)) + Fraction(float(b))) for a, b in zip(d[:, k], Q)])
+        assert_bits_equal(s.cpu().numpy(), S, "sum")
+        assert_bits_equal(q.cpu().numpy(), Q, "sum of squares")
+    else:
+        if form == "interleaved":
+            out = torch.empty((per, n), dtype=torch.float64, device="cuda")
+            rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_INTERLEAVED)
+            got = out.cpu().numpy().T
+        else:
+            if form == "stream_major":
+                rlx.rlxpp_set_chunks(1)  # keep the call on the persistent kernel
+            try:
+                out = torch.empty((n, per), dtype=torch.float64, device="cuda")
+                rlx.rlxpp_generate_doubles(h, out, per, rlx.RLXPP_STREAM_MAJOR)
+            finally:
+                rlx.rlxpp_set_chunks(0)
+            got = out.cpu().numpy()
+        assert np.array_equal((got * 2.0**48).astype(np.uint64), want)
     rlx.rlxpp_destroy(h)
