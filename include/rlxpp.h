@@ -203,6 +203,50 @@ int rlxpp_generate_ragged(rlxpp_t* h, const uint32_t* counts_dev, double* out_de
 int rlxpp_generate_ragged_reduce(rlxpp_t* h, const uint32_t* counts_dev, double* sum_dev, double* sumsq_dev,
                                  int cooperative);
 
+/* ---- Generation for callers that must not allocate device memory -----------------------------------
+ * Who this is for.  Every other way into the generator allocates on the device at some point: rlxpp_create
+ * (state planes, scheduler words, power tables), the first use of a luxury level (its byte matrix), the host
+ * variants (staging buffers).  Some callers cannot afford that, or are not allowed to:
+ *   - code that runs after a framework's memory pool has taken the whole device, where a cudaMalloc from a
+ *     third-party library either fails or goes behind the pool's back;
+ *   - code with a latency budget (a serving loop, a simulation step inside a timed region): cudaMalloc and
+ *     cudaFree synchronise the device and can take milliseconds;
+ *   - code running under a fixed, audited memory plan, where every device byte is accounted for up front.
+ * rlxpp_generate_doubles_static is the one entry point for them: it calls no cudaMalloc, no cudaFree and no
+ * library routine that allocates on the device.  The caller passes the inputs and outputs; everything else the
+ * kernels need -- the 80-byte-per-stream working copy of the states, the scheduler words of the persistent
+ * kernel, the 7,680-byte byte matrix of the luxury level -- lives in ONE fixed array inside the library's
+ * device image (RLXPP_STATIC_SCRATCH_BYTES = 5,255,168 bytes, about 5 MB).  Every GPU that loads librlxpp.so
+ * holds that array from the moment the library's code is loaded on it until the process exits, used or not:
+ * that is the price, and the reason the limit is modest.
+ *
+ * What it computes.  lcg_dev: n_streams LCG states, [n_streams][9] uint64_t (the form rlxpp_get_state exports as
+ * `lcg_dev`; values >= m are reduced first), every stream at a block boundary (cursor 12).  Each stream makes
+ * n_per_stream / 12 advances by A = a^p and its draws (line 39: 12 doubles of 48 bits
+ * per advance) go to out_dev in `layout`, exactly as rlxpp_generate_doubles writes them for a handle holding the
+ * same states; lcg_dev is then overwritten with the advanced states, so that the next call continues the
+ * sequences.  Always the tensor-core kernels (rlxpp_set_engine does not apply); bit-identical with the handle path.
+ *   n_streams <= RLXPP_STATIC_MAX_STREAMS (65,536), else RLXPP_EINVAL ("... exceeds the static scratch ...");
+ *   n_per_stream a multiple of 12 (there is no cursor to keep a partial block in), else RLXPP_EINVAL;
+ *   lcg_dev 8-byte, out_dev 16-byte aligned DEVICE pointers owned by the caller; n_streams == 0 or
+ *   n_per_stream == 0 is a no-op.  Work is enqueued on cuda_stream; the call does not wait for it.
+ *
+ * Set-up.  The FIRST call on each device looks up the array's device address (with that device current) and
+ * uploads the byte matrix; a later call with a DIFFERENT p uploads that level's matrix over it (a copy from
+ * ordinary host memory, enqueued on cuda_stream).  Make the first call on a device -- and the first call for each
+ * new p -- before any stream capture begins.
+ *
+ * Sharing.  There is one array per device and every call uses all of it; it keeps what the last call left there.
+ * The call itself clears the words that must start at zero (scheduler ticket and chunk counters) and rewrites the
+ * state copy from lcg_dev, so nothing carries over between calls.  But two calls that can overlap on the GPU
+ * (different CUDA streams without an event between them, or two host threads) RACE on the array and give wrong
+ * numbers: issue all calls for one device on one stream, or order them yourself.  Handles (rlxpp_create) do not
+ * touch the array and may run alongside. */
+#define RLXPP_STATIC_MAX_STREAMS 65536ull
+#define RLXPP_STATIC_SCRATCH_BYTES 5255168ull
+int rlxpp_generate_doubles_static(uint64_t* lcg_dev, uint64_t n_streams, uint32_t p, double* out_dev,
+                                  uint64_t n_per_stream, int layout, void* cuda_stream);
+
 /* ---- Rare-path counters (debug / test instrumentation of the hot kernels) ------------------------------
  * mod_m ("smaller than m in all cases") and the conversion back to RANLUX numbers (line 39)
  * run in the hot kernels as fast forms that take the overwhelmingly likely case and hand everything else to

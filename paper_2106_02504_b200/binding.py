@@ -19,6 +19,8 @@ RLXPP_AOS = 0
 RLXPP_SOA = 1
 RLXPP_ENGINE_UMMA = 0
 RLXPP_ENGINE_IMAD = 1
+RLXPP_STATIC_MAX_STREAMS = 65536
+RLXPP_STATIC_SCRATCH_BYTES = 5255168
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librlxpp.so")
@@ -55,6 +57,8 @@ _SIGNATURES = {
     "rlxpp_generate_u48": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
     "rlxpp_generate_floats": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
     "rlxpp_generate_normal": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]),
+    "rlxpp_generate_doubles_static": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_void_p,
+                                                     ctypes.c_uint64, ctypes.c_int, ctypes.c_void_p]),
     "rlxpp_host_generate": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64,
                                            ctypes.c_uint64, ctypes.c_void_p]),
     "rlxpp_device_view": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
@@ -190,6 +194,15 @@ def rlxpp_generate_floats(h: Handle, out_dev, n_per_stream: int, layout: int = R
 
 def rlxpp_generate_normal(h: Handle, out_dev, n_per_stream: int, layout: int = RLXPP_STREAM_MAJOR):
     _check(load().rlxpp_generate_normal(h.ptr, _ptr(out_dev), n_per_stream, layout), "rlxpp_generate_normal")
+
+
+def rlxpp_generate_doubles_static(lcg_dev, n_streams: int, p: int, out_dev, n_per_stream: int,
+                                  layout: int = RLXPP_STREAM_MAJOR, cuda_stream=None):
+    """The generator for callers that must not allocate device memory (include/rlxpp.h): states in, doubles and
+    advanced states out, scratch in the library's own fixed device array (at most RLXPP_STATIC_MAX_STREAMS streams)."""
+    s = _current_stream() if cuda_stream is None else cuda_stream
+    _check(load().rlxpp_generate_doubles_static(_ptr(lcg_dev), n_streams, p, _ptr(out_dev), n_per_stream, layout, s),
+           "rlxpp_generate_doubles_static")
 
 
 def rlxpp_host_generate(lcg: np.ndarray, pos: int, p: int, skip: int, n: int):

@@ -490,6 +490,67 @@ static int check_device() {
   return RLXPP_OK;
 }
 
+// ----------------------------------------------------------------------------- rlxpp_generate_doubles_static
+// The scratch of the one entry point that allocates nothing (include/rlxpp.h says who needs that and why).  It is
+// part of the library's device image: each GPU gets its own copy when the image is loaded there and keeps it until
+// the process ends.  Layout, all offsets multiples of 256 bytes:
+//   [kStaticBmat,  + 8 KB)   byte matrix of the luxury level last used on this device (tc::kBBytes = 7,680)
+//   [kStaticSched, + 4 KB)   scheduler words of the persistent kernel: ticket + one chunk counter per tile (<= 513)
+//   [kStaticState, + 5 MB)   the five state planes of up to RLXPP_STATIC_MAX_STREAMS streams (80 bytes each)
+// In HOST code `g_static_scratch` is only a stand-in the runtime knows the symbol by -- not a device address; handing
+// it to a kernel would fault, or quietly use the wrong memory.  static_scratch_base() asks the runtime for the real
+// address, once per device, with that device current.
+constexpr size_t kStaticBmat = 0, kStaticSched = 8192, kStaticState = 12288;
+constexpr size_t kStaticBytes = kStaticState + 5 * sizeof(uint4) * RLXPP_STATIC_MAX_STREAMS;
+static_assert(kStaticBytes == RLXPP_STATIC_SCRATCH_BYTES, "rlxpp.h states the size of the static scratch");
+static_assert(tc::kBBytes <= kStaticSched - kStaticBmat, "byte matrix does not fit its slot");
+static_assert((1 + (RLXPP_STATIC_MAX_STREAMS + tc::kTile - 1) / tc::kTile) * sizeof(uint32_t) <= kStaticState - kStaticSched,
+              "scheduler words do not fit their slot");
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+struct StaticDev {
+  unsigned char* base = nullptr;  // device address of g_static_scratch on this device
+  uint32_t p_loaded = 0;          // luxury level whose byte matrix sits at kStaticBmat (0 = none yet)
+};
+static std::mutex g_static_mutex;
+static StaticDev g_static_dev[64];
+
+// Host images of the byte matrices, one per p, never freed: the upload below reads them asynchronously.
+static const std::vector<uint8_t>& static_bmatrix_image(uint32_t p) {
+  static std::vector<std::pair<uint32_t, std::vector<uint8_t>*>> cache;  // under g_static_mutex
+  for (const auto& e : cache)
+    if (e.first == p) return *e.second;
+  std::vector<uint8_t>* img = new std::vector<uint8_t>();
+  build_bmatrix(p, *img);
+  cache.emplace_back(p, img);
+  return *img;
+}
+
+// Set-up of the static scratch for the CURRENT device and luxury level p: address look-up on the device's first call,
+// matrix upload (stream-ordered on s) whenever p changes.  No device allocation.
+static int static_scratch_base(uint32_t p, cudaStream_t s, unsigned char** out) {
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(RLXPP_EINVAL, "rlxpp_generate_doubles_static: device ordinal %d not in [0, 64)", dev);
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticDev& d = g_static_dev[dev];
+  if (!d.base) {
+    unsigned char* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_static_scratch);
+    if (e != cudaSuccess || !ptr)
+      return fail(RLXPP_ECUDA, "rlxpp_generate_doubles_static: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+    d.base = ptr;
+  }
+  if (d.p_loaded != p) {
+    const std::vector<uint8_t>& img = static_bmatrix_image(p);
+    d.p_loaded = 0;  // unknown contents if the copy fails half way
+    CUDA_TRY(cudaMemcpyAsync(d.base + kStaticBmat, img.data(), tc::kBBytes, cudaMemcpyHostToDevice, s));
+    d.p_loaded = p;
+  }
+  *out = d.base;
+  return RLXPP_OK;
+}
+
 extern "C" {
 
 const char* rlxpp_last_error(void) { return g_last_error.c_str(); }
@@ -833,6 +894,45 @@ int rlxpp_generate_floats(rlxpp_t* h, float* out_dev, uint64_t n_per_stream, int
 
 int rlxpp_generate_normal(rlxpp_t* h, double* out_dev, uint64_t n_per_stream, int layout) {
   return generate_other(h, out_dev, n_per_stream, layout, kNormal, "rlxpp_generate_normal");
+}
+
+// Generation for callers that must not allocate on the device (include/rlxpp.h has the contract and the reasons): the
+// same import -> persistent tensor-core kernel -> export sequence a handle would run, with the handle's device buffers
+// replaced by slices of g_static_scratch.  Nothing below may call cudaMalloc / cudaFree or a routine that does --
+// which rules out get_bmatrix(), cached_tables()'s device copies and the time-parallel path (lane_sync stays null).
+int rlxpp_generate_doubles_static(uint64_t* lcg_dev, uint64_t n_streams, uint32_t p, double* out_dev, uint64_t n_per_stream,
+                                  int layout, void* cuda_stream) {
+  const char* who = "rlxpp_generate_doubles_static";
+  if (p == 0) return fail(RLXPP_EINVAL, "%s: p == 0", who);
+  if (layout != RLXPP_STREAM_MAJOR && layout != RLXPP_INTERLEAVED) return fail(RLXPP_EINVAL, "%s: unknown layout %d", who, layout);
+  if (n_streams > RLXPP_STATIC_MAX_STREAMS)
+    return fail(RLXPP_EINVAL, "%s: %llu streams exceeds the static scratch, which holds at most %llu (use rlxpp_create for more)", who,
+                (unsigned long long)n_streams, (unsigned long long)RLXPP_STATIC_MAX_STREAMS);
+  if (n_per_stream % 12)
+    return fail(RLXPP_EINVAL, "%s: n_per_stream = %llu is not a multiple of 12 (whole blocks only)", who, (unsigned long long)n_per_stream);
+  if (n_streams == 0 || n_per_stream == 0) return RLXPP_OK;
+  if (!lcg_dev || !out_dev) return fail(RLXPP_EINVAL, "%s: null states or output", who);
+  if ((uintptr_t)lcg_dev % 8 || (uintptr_t)out_dev % 16) return fail(RLXPP_EINVAL, "%s: states must be 8-byte, output 16-byte aligned", who);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  unsigned char* base = nullptr;
+  int rc = static_scratch_base(p, s, &base);  // first call on this device: address look-up; new p: matrix upload
+  if (rc) return rc;
+  uint4* planes = reinterpret_cast<uint4*>(base + kStaticState);
+  // every word of the planes that the kernels read is rewritten here, so the last call's states never show through
+  import_kernel<<<grid_for(n_streams), kThreads, 0, s>>>(planes, n_streams, lcg_dev, nullptr);
+  LAUNCH_CHECK();
+  GenArgs a;
+  a.st = planes; a.n_total = n_streams; a.first = 0; a.count = n_streams; a.out = out_dev; a.ld = n_streams;
+  a.n_per = n_per_stream; a.sum = nullptr; a.sumsq = nullptr; a.p = p;
+  host::multiplier_ap(p).to_u32x18(a.A.v);
+  a.bmat = reinterpret_cast<const uint4*>(base + kStaticBmat);
+  a.sched = reinterpret_cast<uint32_t*>(base + kStaticSched);  // zeroed by the launch below (cudaMemsetAsync), every call
+  rc = layout == RLXPP_STREAM_MAJOR ? launch_tc_generate_mode<kStoreStreamMajor>(a, true, s)
+                                    : launch_tc_generate_mode<kStoreInterleaved>(a, true, s);
+  if (rc) return rc;
+  export_kernel<<<grid_for(n_streams), kThreads, 0, s>>>(planes, n_streams, nullptr, nullptr, nullptr, lcg_dev);
+  LAUNCH_CHECK();
+  return RLXPP_OK;
 }
 
 static int ensure_staging(rlxpp_t* h, size_t bytes_each) {
