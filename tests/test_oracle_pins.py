@@ -333,6 +333,27 @@ def test_stream_draws_match_bigint_model_and_survey_vectors(oracle):
         assert [int(v) for v in got] == py_stream(seed, p, 40)
 
 
+def test_stream_end_states_match_bigint_model(oracle):
+    """The X / V / c / pos arrays oracle.streams returns with want=("state",) -- what every GPU check_state compares
+    with -- against Python integers: after `skip` skipped and n taken draws from pos = 12 the stream has made
+    k = ceil((skip + n) / 12) advances (D8), X = A^k X0, V = floor(2^576 X / m) (D4 by its definition, not the shift / add
+    form) and c = X - V + (V >> 336) (D3 solved for the carry), cursor = skip + n - 12 (k - 1)."""
+    for p, seed_list, n, skip_list in ((2048, (1, 2, 77), 29, (0, 5, 1000)), (2048, (3, 4), 36, (0, 12)),
+                                       (24, (9, 2**64 - 1), 1, (0, 11)), (389, (5,), 0, (7,))):
+        r = oracle.streams(np.array(seed_list, np.uint64), p, n, skips=np.array(skip_list, np.uint64), want=("state",))
+        A = pow(A1, p, M)
+        for i, (seed, skip) in enumerate(zip(seed_list, skip_list)):
+            total = skip + n
+            k = (total + 11) // 12
+            X = pow(A, k, M) * pow(A, seed << 96, M) % M
+            V = (X << 576) // M
+            c = X - V + (V >> 336)
+            assert c in (0, 1)
+            assert inputs.limbs_to_int(r["X"][i]) == X, (p, seed, skip)
+            assert inputs.limbs_to_int(r["V"][i]) == V, (p, seed, skip)
+            assert int(r["c"][i]) == c and int(r["pos"][i]) == (total - 12 * (k - 1) if total else 12)
+
+
 def test_cfg1_checksums(oracle):
     """BASELINE.json configs[0]: 1,024 streams x 384 draws, seeds 1..1024, p = 2048."""
     r = oracle.streams(inputs.seeds(1024), 2048, 384, want=("ints", "doubles", "state"), nthreads=4)
