@@ -422,7 +422,7 @@ def main():
         wpeak = SM_COUNT * 4 * sm_max_mhz * 1e6 / 1e9
         roofline = {"bound": "alu", "kernel": kernel.replace("aligned>", "aligned, normal>"), "achieved": winst, "peak": wpeak,
                     "unit": "G warp instructions/s", "frac": winst / wpeak, "traffic": None,
-                    "peak_source": f"{WARP_INST_PER_ADVANCE["normal"]} warp instructions per advance of 32 streams (ncu, "
+                    "peak_source": f"{WARP_INST_PER_ADVANCE['normal']} warp instructions per advance of 32 streams (ncu, "
                                    f"smsp__inst_executed) x advances; peak = {SM_COUNT} SMs x 4 schedulers x {sm_max_mhz:.0f} MHz",
                     "kernel_ms": kernel_ms, "alu": alu, "hbm": hbm}
     roofline["engine"] = args.engine
@@ -488,6 +488,28 @@ def main():
         compare = {"engine": other, "value": units / (c0.elapsed_time(c1) / 3 * 1e-3), "unit": UNIT, "steps": 3,
                    "n_gpus": 1, "what": "same workload and launch configuration with the other engine, this rank only"}
         rlx.rlxpp_set_engine(engines[args.engine])
+
+    # ---------------------------------------------------------------- cfg5 with its skip-ahead inside the timed region
+    # BASELINE.json configs[4] is "skip-ahead PLUS fused consumption".  `value` above times the fused generation alone (the
+    # skip is one call before the first step, as in the paper's use: seed / skip once, then draw); this leg times
+    # rlxpp_skip_each (random 64-bit distances: ~32 generic modular products per stream) + rlxpp_generate_reduce per step.
+    with_skip = None
+    if args.workload == "cfg5" and rank == 0:
+        def skip_step():
+            rlx.rlxpp_skip_each(h, sk)
+            step()
+        skip_step()
+        torch.cuda.synchronize()
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record(stream)
+        for _ in range(args.steps):
+            skip_step()
+        k1.record(stream)
+        torch.cuda.synchronize()
+        ws_ms = k0.elapsed_time(k1) / args.steps
+        with_skip = {"value": units / (ws_ms * 1e-3), "unit": UNIT, "ms_per_step": ws_ms, "steps": args.steps, "n_gpus": 1,
+                     "skip_share_of_step": 1.0 - kernel_ms / ws_ms,
+                     "what": "rlxpp_skip_each (seeded random 64-bit distance per stream) + rlxpp_generate_reduce per step, this rank"}
 
     # ---------------------------------------------------------------- sustained: the same step for >= 3 s
     sustained = None
@@ -620,6 +642,14 @@ def main():
             "clocks": clocks,
             "other_engine": compare,
         }
+        if with_skip is not None:
+            line["with_skip"] = with_skip
+            line["config"]["timed_step"] = ("rlxpp_generate_reduce only; the per-stream skip runs once before the first step "
+                                            "(`with_skip` has both inside the timed region)")
+        if args.workload == "cfg2":
+            line["config"]["deferred_fold"] = True
+            line["config"]["timed_step"] = (f"{n_per} products + 1 fold per state: between repetitions the state stays an "
+                                            "unreduced product (< 2^591), mod_m runs once at the end; same canonical result")
         if devapi is not None:
             devapi["random_cursors_tile"] = value
             line["device_api"] = devapi

@@ -204,6 +204,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_lanes_k
     const uint4* src = a.bmat_pow + (u64)(K - 1) * (tc::kBBytes / 16);
     uint4* dst = reinterpret_cast<uint4*>(bstride);
     for (u32 q = threadIdx.x; q < tc::kBBytes / 16; q += tc::kTile) dst[q] = __ldg(src + q);
+    umma::fence_proxy_async_smem();  // read by tcgen05.mma (async proxy) after the CTA barrier in tile.setup()
   }
   tc::Tile<tc::kSyncCta> tile;
   tile.setup(smem, a.bmat_pow + (u64)lane * (tc::kBBytes / 16));  // the matrix of A^(lane + 1)
@@ -221,7 +222,7 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_lanes_k
   if (MODE == kStoreStreamMajor) sink.p = a.out + il * (a.pitch ? a.pitch : a.n_per);
   else if (OUT == kF32) sink.p = reinterpret_cast<double*>(reinterpret_cast<float*>(a.out) + il);
   else sink.p = a.out + il;
-  tile.issue(x);  // (CTA barrier inside: every thread's state now sits in shared memory)
+  tile.issue(x);  // (CTA barrier inside: every thread has read its state and written it to the A operand in tensor memory)
   if (threadIdx.x == 0) {
     __threadfence();
     atomicAdd(a.lane_sync + tidx, 1u);  // this lane has read the tile's state
@@ -241,6 +242,8 @@ __global__ void __launch_bounds__(tc::kTile, tc::kCtasPerSm) tc_generate_lanes_k
         do {
           asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(readers) : "l"(a.lane_sync + tidx) : "memory");
         } while (readers < K);
+        // back to zero for the next launch: a plain store is enough, the only later reader is a later launch on the
+        // handle's stream (kernel boundaries order it); no CTA of THIS grid touches the word after its own atomicAdd
         a.lane_sync[tidx] = 0;
       }
       __syncthreads();

@@ -290,7 +290,9 @@ struct RingStage {
 // stores are 24 instructions of 128 bytes per warp and advance (measured 700 G draws/s).  Instead the CTA parks a
 // block as [24 float rows][128 streams] in shared memory and ONE thread of the MMA-issuing warp hands it to the TMA
 // as a box of 24 rows x 512 bytes.  No new barrier: the box of block b - 1 is sent from Tile::issue() of advance
-// b + 1, where every thread has fenced its stores and arrived at the hand-off barrier anyway.  Ring of three boxes:
+// b + 1, after the hand-off barrier every thread arrives at anyway.  Tile::issue() no longer fences (its A operand
+// moved to tensor memory), so emit() itself ends with fence.proxy.async.shared::cta in every thread: the floats a
+// thread parked are ordered before the barrier, and through it before the sender's cp.async.bulk.  Ring of three boxes:
 // block b is written after collect() of advance b, i.e. after the MMA-done mbarrier that the issuing thread committed
 // AFTER waiting (cp.async.bulk.wait_group.read) for the copy of block b - 3.
 constexpr u32 kF32BoxBytes = 24u * 128u * 4u;               // 12,288
@@ -324,6 +326,7 @@ struct F32RowStage {
   }
   __device__ __forceinline__ void emit(const u32 (&v)[18]) {
     park<0>(base + (nfilled % 3u) * kF32BoxBytes + col, v);
+    umma::fence_proxy_async_smem();  // generic-proxy stores above -> async-proxy read by the TMA in send_parked()
     nfilled++;
   }
   // issuing warp, before the MMAs: the boxes sent so far have been read
@@ -331,7 +334,7 @@ struct F32RowStage {
     if (sender) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     __syncwarp();
   }
-  // the CTA's stores to the parked blocks are fenced and handed over: send what is parked and unsent
+  // every thread fenced its parked floats in emit() and has passed the hand-off barrier: send what is parked and unsent
   __device__ __forceinline__ void send_parked() {
     if (sender) {
       while (nsent < nfilled) {

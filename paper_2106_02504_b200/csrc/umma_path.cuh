@@ -91,6 +91,9 @@ struct Tile {
     const u32 tid = threadIdx.x;
     uint4* sb = reinterpret_cast<uint4*>(s.b);
     for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
+    // B was written with ordinary (generic-proxy) stores and tcgen05.mma reads it through its shared-memory descriptor,
+    // i.e. through the async proxy: every thread fences what it wrote, the barrier below hands it to the issuing thread
+    umma::fence_proxy_async_smem();
     bar = umma::smem_u32(&s.bar);
     phase = 0;
     if (tid == 0) {
@@ -115,9 +118,12 @@ struct Tile {
   __device__ __forceinline__ void issue(const u32 (&x)[18]) {
     issue(x, [] {}, [] {});
   }
-  // before() / after() run in the ISSUING warp (all of its lanes), after the whole CTA has fenced and handed over what
-  // it stored to shared memory, right before and right after the MMAs are issued and committed: the place for other
-  // async-proxy work on the CTA's shared memory that must be ordered with the MMA-done mbarrier (F32RowStage).
+  // before() / after() run in the ISSUING warp (all of its lanes), after the hand-off barrier, right before and right
+  // after the MMAs are issued and committed: the place for other async-proxy work on the CTA's shared memory that must be
+  // ordered with the MMA-done mbarrier (F32RowStage).  The A operand lives in tensor memory, so issue() itself executes
+  // NO proxy fence: a caller whose after() lets the TMA read shared memory must have had every writing thread execute
+  // fence.proxy.async.shared::cta BEFORE calling issue() (F32RowStage::emit does, right after parking its floats); the
+  // hand-off barrier then orders those fenced writes before the sender's cp.async.bulk.
   template <class Before, class After>
   __device__ __forceinline__ void issue(const u32 (&x)[18], Before&& before, After&& after) {
     umma::tmem_st18(tld + kACol, x);
@@ -207,6 +213,9 @@ struct PairTile {
     ticket = &s.ticket;
     uint4* sb = reinterpret_cast<uint4*>(s.b);
     for (u32 q = tid; q < kBBytes / 16; q += kTile) sb[q] = __ldg(bmat + q);
+    // B was written with ordinary (generic-proxy) stores and tcgen05.mma reads it through its shared-memory descriptor,
+    // i.e. through the async proxy: every thread fences what it wrote, the barrier below hands it to the issuing thread
+    umma::fence_proxy_async_smem();
     bar = umma::smem_u32(&s.bar);
     phase = 0;
     if (tid == 0) {
@@ -442,7 +451,8 @@ struct GroupTile {
   __device__ __forceinline__ void teardown() {
     umma::fence_before_sync();
     __syncthreads();
-    if (threadIdx.x < 32) umma::tmem_dealloc(tmem, 512u);
+    // the allocation's own base (group 0's `tmem` happens to equal it, but the dealloc must not depend on that)
+    if (threadIdx.x < 32) umma::tmem_dealloc(tmem - (threadIdx.x / kTile) * kGroupCols, 512u);
   }
 };
 
