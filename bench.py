@@ -251,6 +251,10 @@ def main():
                          "48-bit draws per second")
     ap.add_argument("--chunks", type=int, default=0,
                     help="UMMA engine: force the number of chunks per tile (rlxpp_set_chunks; 0 = the library decides)")
+    ap.add_argument("--streams", type=int, default=0,
+                    help="streams per GPU instead of the workload's (A/B runs and small multi-process dry runs; the line's "
+                         "config.workload then carries the shape)")
+    ap.add_argument("--per-stream", type=int, default=0, help="doubles per stream instead of the workload's")
     ap.add_argument("--no-compare", action="store_true", help="skip the short run of the other engine")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle cpu_baseline leg")
@@ -286,6 +290,10 @@ def main():
     n_streams, n_per, p, desc = WORKLOADS[args.workload]
     if args.p:
         p = args.p
+    if args.streams or args.per_stream:  # not a BASELINE configuration any more: say so where the workload is named
+        n_streams, n_per = args.streams or n_streams, args.per_stream or n_per
+        desc = f"{args.workload} kernels on another shape: {n_streams} streams x {n_per} doubles (--streams / --per-stream)"
+        args.no_cpu = True  # the oracle leg and its sample sizes are defined for the BASELINE shapes only
     # weak scaling: the job has world x n_streams streams, rank g owns the contiguous range g
     first_stream, my_streams, first_seed = job_layout(rank, world, n_streams)
     assert my_streams == n_streams
@@ -630,7 +638,7 @@ def main():
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": ("u8 x u8 -> s32 (tcgen05.mma kind::i8) + u32 limbs -> f64" if umma
                       else "u32 limbs (IMAD.WIDE.U32, 64-bit accumulate) -> f64"), "data": "synthetic",
-            "config": {"workload": args.workload, "engine": args.engine, "layout": args.layout, "output": args.output, "description": desc, "n_streams_per_gpu": n_streams,
+            "config": {"workload": args.workload if not (args.streams or args.per_stream) else f"{args.workload}-shape {n_streams} x {n_per}", "engine": args.engine, "layout": args.layout, "output": args.output, "description": desc, "n_streams_per_gpu": n_streams,
                        "doubles_per_stream": n_per, "p": p, "l2": "output per step (12.9 GB) exceeds L2; no flush needed"
                        if args.workload in ("cfg3", "cfg4") else ("3 MB of output: L2-resident, launch-latency bound"
                                                                   if args.workload == "cfg1" else

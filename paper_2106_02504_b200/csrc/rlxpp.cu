@@ -245,25 +245,35 @@ static int launch_generate_mult(const GenArgs& a, int mode, bool aligned, cudaSt
     default: return launch_generate_mode<Mult, kReduce>(a, aligned, s);
   }
 }
-// Work items of the persistent UMMA kernel: how many chunks to cut every tile's n_per draws into so
-// that the last, partial wave of the grid is short.  One chunk unless the tiles alone fill the
-// resident CTAs badly; a chunk is never shorter than 16 advances (state I/O and pipeline fill).
-static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_t* n_chunks, uint64_t* chunk_len) {
+// Work items of the persistent UMMA kernel: how many chunks to cut every tile's n_per draws into.  One chunk unless the
+// tiles alone fill the resident CTAs badly; a chunk is never shorter than 16 advances (state I/O and pipeline fill).
+//   Store kernels (hbm_bound): the CTAs of a wave start together and, all waiting on the same HBM, stay in step, so every
+//   wave boundary is a bubble in the write stream that no other CTA fills, while a ragged last wave costs little (the
+//   CTAs still running get the bandwidth of those that finished).  Fewest chunks that give >= 6.5 items per resident
+//   CTA (items of two tiles; 13 where an item is one tile): measured round 3 (profiles/ab_r03_chunks.md) cfg3 787 -> 827 G doubles/s with 1 chunk instead of 2; within 2 %
+//   of the best chunk count on every shape tried (2^18 .. 2^21 streams x 768 .. 6,144 draws).
+//   Fused reduce (ALU-bound): CTAs run at their own pace and the last wave counts in full: >= 97 % fill and >= 12 waves.
+static void plan_items(uint64_t n_tiles, uint64_t n_per, unsigned slots, uint32_t* n_chunks, uint64_t* chunk_len, bool hbm_bound,
+                       bool pairs) {
   *n_chunks = 1;
   *chunk_len = n_per;
   const uint64_t blocks = n_per / 12;
   if (n_tiles <= slots || blocks < 32) return;
-  // a good plan fills >= 97 % of its last wave AND has >= 12 waves: CTAs do not run at equal speed when the
-  // kernel is HBM-bound, and finer items even that out (cfg4: 2 chunks 764, 4 chunks 793 G doubles/s at the
-  // same 98.8 % fill; profiles/ab_r01_sync.md)
-  double best = 0.0;
   uint64_t best_c = 1;
-  for (uint64_t c = 1; c <= 16 && blocks / c >= 16; c++) {
-    const uint64_t items = n_tiles * c, waves = (items + slots - 1) / slots;
-    const double eff = (double)items / (double)(waves * slots);
-    const double score = eff - (waves < 12 ? 0.05 : 0.0);
-    if (score > best + 1e-9) { best = score; best_c = c; }
-    if (eff >= 0.97 && waves >= 12) break;
+  if (hbm_bound) {
+    const uint64_t want = pairs ? ((uint64_t)slots * 13 + 1) / 2 : (uint64_t)slots * 13;  // 6.5 items of two tiles per resident CTA, or 13 of one
+    best_c = (want + n_tiles - 1) / n_tiles;
+    if (best_c > 16) best_c = 16;
+    while (best_c > 1 && blocks / best_c < 16) best_c--;
+  } else {
+    double best = 0.0;
+    for (uint64_t c = 1; c <= 16 && blocks / c >= 16; c++) {
+      const uint64_t items = n_tiles * c, waves = (items + slots - 1) / slots;
+      const double eff = (double)items / (double)(waves * slots);
+      const double score = eff - (waves < 12 ? 0.05 : 0.0);
+      if (score > best + 1e-9) { best = score; best_c = c; }
+      if (eff >= 0.97 && waves >= 12) break;
+    }
   }
   if (best_c == 1) return;
   const uint64_t len = ((blocks + best_c - 1) / best_c + 7) / 8 * 96;  // whole cycles of 8 blocks (StreamMajorStage)
@@ -419,7 +429,7 @@ static int launch_tc_generate_mode(GenArgs a, bool aligned, cudaStream_t s) {
       return RLXPP_OK;
     }
   }
-  plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len);
+  plan_items(n_tiles, a.n_per, slots, &a.n_chunks, &a.chunk_len, MODE != kReduce, kPairs);
   if (g_force_chunks.load() > 0 && a.n_per / 12 >= (uint64_t)g_force_chunks.load()) {  // test hook
     const uint64_t c = (uint64_t)g_force_chunks.load(), blocks = a.n_per / 12;
     a.chunk_len = ((blocks + c - 1) / c + 7) / 8 * 96;
