@@ -467,6 +467,9 @@ def main():
             roofline["imad_microbench_peak"] = rlx.rlxpp_measure_imad_peak(3) / 1e9
             roofline["frac_of_imad_microbench"] = imad_achieved / 1e9 / roofline["imad_microbench_peak"]
             roofline["hbm_write_microbench_peak"] = rlx.rlxpp_measure_hbm_write_peak(8 << 30, 3) / 1e9
+            # the write-only denominator next to the driver's copy figure (a copy reads as much as it writes; a kernel
+            # that only writes can exceed it): the kernel's own store pattern without its arithmetic
+            roofline["frac_of_hbm_write_microbench"] = hbm_achieved / roofline["hbm_write_microbench_peak"]
         except rlx.RlxppError as e:  # the probes are context, the headline does not depend on them
             roofline["probe_error"] = str(e)
     traffic_file = os.path.join(ROOT, TRAFFIC_FILE)

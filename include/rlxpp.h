@@ -282,7 +282,9 @@ uint64_t rlxpp_launch_count(void);
 /* Roofline denominators measured on the device the caller is on:
  *   imad: a dependency-free stream of IMAD.WIDE.U32.X (carry-chained, 64-bit accumulate)
  *         issued from every SM; returns multiply-accumulates per second.
- *   hbm_write: a write-only kernel storing `bytes` bytes with 128-bit stores; bytes/s.
+ *   hbm_write: write-only kernels storing `bytes` bytes: a grid-stride sweep of 128-bit stores, and (for >= 1.5 GiB)
+ *         the interleaved generate kernels' own pattern without their arithmetic -- strips of 256 doubles of 2 MB rows,
+ *         256 contiguous bytes per warp store, walking down the rows; the better of the two in bytes/s.
  * Both time `iters` launches with CUDA events after a warm-up and report the best. */
 int rlxpp_measure_imad_peak(int iters, double* imad_per_s, void* cuda_stream);
 int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s, void* cuda_stream);

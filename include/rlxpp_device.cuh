@@ -593,7 +593,11 @@ class StreamT {
     detail::to_ranlux_fast(x, v, c, rare);  // decides the carry from two leading words; exact form otherwise (~2^-16)
     if (__builtin_expect(rare != 0, 0)) detail::to_ranlux_exact(x, v, c);
   }
-  // draw number pos_ of the current block: bits [48 pos, 48 pos + 48) of V
+  // draw number pos_ of the current block: bits [48 pos, 48 pos + 48) of V.  v_[w] with a run-time w keeps the block in
+  // local memory (L1-resident: 18 stores per advance, two loads per draw).  A 12-way switch with compile-time indices
+  // keeps it in registers (0 bytes of stack) but measured SLOWER in round 3: aligned draw 245 -> 233, draw_coop
+  // 209 -> 186, draw_coop with random cursors 116 -> 76 G doubles/s (up to 30 more registers, and the switch diverges
+  // when the cursors differ) -- the indexed form stays.
   __device__ __forceinline__ uint64_t take() {
     const uint32_t w = (3u * pos_) >> 1;  // 32-bit word holding bit 48 pos
     uint64_t k;

@@ -256,6 +256,24 @@ __global__ void __launch_bounds__(256) hbm_write_kernel(uint4* __restrict__ out,
   for (u64 q = (u64)blockIdx.x * blockDim.x + threadIdx.x; q < n16; q += stride) __stcs(out + q, val);
 }
 
+// The write-only ceiling for the pattern the interleaved generate kernels produce (tc_pair_kernel), without their
+// arithmetic: a persistent grid of 128-thread CTAs, an item = a strip of 256 columns x `rows_per_item` rows of a row-major
+// array of doubles with `ld` columns; per row the warp stores 256 contiguous bytes twice (the two tiles of a pair),
+// streaming (st.global.cs), and walks down the rows.  Items are dealt round-robin: strips of one chunk of rows first.
+__global__ void __launch_bounds__(128, 4) hbm_write_rows_kernel(double* __restrict__ out, u64 ld, u64 n_rows, u32 rows_per_item) {
+  const u64 strips = ld / 256, chunks = (n_rows + rows_per_item - 1) / rows_per_item;
+  const double v = __longlong_as_double(0x3ff0000000000000ll | (long long)threadIdx.x);
+  for (u64 w = blockIdx.x; w < strips * chunks; w += gridDim.x) {
+    const u64 strip = w % strips, r0 = (w / strips) * rows_per_item;
+    const u64 r1 = r0 + rows_per_item < n_rows ? r0 + rows_per_item : n_rows;
+    double* p = out + r0 * ld + strip * 256 + threadIdx.x;
+    for (u64 r = r0; r < r1; r++, p += ld) {
+      __stcs(p, v);
+      __stcs(p + 128, v);
+    }
+  }
+}
+
 // Store-pattern probe (rlxpp_measure_hbm_write_pieces): what a stream-major output looks like to the
 // memory system.  Every warp of a persistent grid owns 32 rows at a time and walks along them, writing
 // one piece of `piece16` x 16 bytes of each of its rows per step with full 128-bit stores.

@@ -1232,6 +1232,22 @@ int rlxpp_measure_hbm_write_peak(uint64_t bytes, int iters, double* bytes_per_s,
     const double rate = (double)(bytes / 16 * 16) / (ms * 1e-3);
     if (it >= 2 && rate > best) best = rate;
   }
+  // second pattern: rows of 2^18 doubles written strip by strip as the interleaved generate kernels write them
+  // (hbm_write_rows_kernel); the result is the better of the two
+  const u64 ld = 1ull << 18, n_rows = bytes / (ld * sizeof(double));
+  if (n_rows >= 768) {
+    for (int it = 0; it < iters + 2; it++) {
+      CUDA_TRY(cudaEventRecord(e0, s));
+      hbm_write_rows_kernel<<<tc_slots(), 128, 0, s>>>(reinterpret_cast<double*>(buf), ld, n_rows, 768u);
+      g_launches++;
+      CUDA_TRY(cudaEventRecord(e1, s));
+      CUDA_TRY(cudaEventSynchronize(e1));
+      float ms = 0.f;
+      CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+      const double rate = (double)(n_rows * ld * sizeof(double)) / (ms * 1e-3);
+      if (it >= 2 && rate > best) best = rate;
+    }
+  }
   *bytes_per_s = best;
   return RLXPP_OK;
 }
