@@ -31,7 +31,7 @@ IMAD_PER_DOUBLE = 27    # 324 / 12 (one LCG operation per 12 
 # (advances / 32) of the committed --set full captures; profiles/ncu_r02_umma.md).  The issue-slot roofline of the
 # kernels that neither HBM nor the tensor pipe binds: one warp instruction per scheduler and clock.
 WARP_INST_PER_ADVANCE = {"normal": 813, "cfg5": 216, "cfg2": 158}
-TRAFFIC_FILE = "profiles/traffic_r02.json"
+TRAFFIC_FILE = "profiles/traffic_r03.json"
 SM_COUNT = 148
 IMAD_LANES_PER_CLK_SM = 64  # fma-heavy pipe: one warp instruction per 2 cycles per SMSP, 4 SMSPs
 
