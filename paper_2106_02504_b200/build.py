@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librlxpp.so")
 SOURCES = ["rlxpp.cu"]
 DEPS = ["rlxpp.cu", "arith.cuh", "state.cuh", "emit.cuh", "stages.cuh", "kernels_imad.cuh", "kernels_umma.cuh", "kernels_misc.cuh",
-        "umma.cuh", "umma_path.cuh", "host_bigint.h", os.path.join("..", "..", "include", "rlxpp_rows.cuh"), "gen_rows.py", "normal_coeffs.cuh",
+        "umma_path.cuh", "host_bigint.h", os.path.join("..", "..", "include", "rlxpp_rows.cuh"), "gen_rows.py", "normal_coeffs.cuh",
         os.path.join("..", "..", "include", "rlxpp.h"), os.path.join("..", "..", "include", "rlxpp_device.cuh"),
         os.path.join("..", "..", "include", "rlxpp_tile.cuh")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -17,6 +17,10 @@
 
 namespace rlx {
 
+// the PTX wrappers of the tensor-core path (tcgen05 / TMEM / mbarrier / proxy fences) live in the public header too,
+// shared by the library's kernels and by rlxpp_dev::TileStream
+namespace umma = rlxpp_dev::umma;
+
 using rlxpp_dev::detail::u32;
 using rlxpp_dev::detail::u64;
 using rlxpp_dev::detail::i64;

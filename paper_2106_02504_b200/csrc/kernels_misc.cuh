@@ -3,6 +3,7 @@
 #pragma once
 
 #include "state.cuh"
+#include "kernels_imad.cuh"  // load_raw / store_raw: the AoS stage of the raw states
 
 namespace rlx {
 
@@ -56,35 +57,58 @@ __global__ void __launch_bounds__(kThreads) skip_kernel(uint4* __restrict__ st, 
   if (live) store_state(st, n, i, x, newpos);
 }
 
-// get_state: the paper's stored form: packed RANLUX numbers + carry, cursor, LCG state
+// get_state: the paper's stored form: packed RANLUX numbers + carry, cursor, LCG state.  The [n][9] uint64 arrays
+// are AoS with a 72-byte stride per stream: 16-byte aligned arrays go through the raw-state stage of kernels_imad.cuh (the
+// CTA's 128 states are 9,216 contiguous bytes: 128-bit coalesced accesses, each thread picks up its 72 bytes in shared
+// memory); other alignments keep the direct per-thread accesses.
+__device__ __forceinline__ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+__device__ __forceinline__ void store_u64x9(u64* __restrict__ dst, u64 i, const u32 (&w)[18]) {
+#pragma unroll
+  for (int l = 0; l < 9; l++) dst[i * 9 + l] = (u64)w[2 * l] | ((u64)w[2 * l + 1] << 32);
+}
 __global__ void __launch_bounds__(kThreads) export_kernel(const uint4* __restrict__ st, u64 n, u64* __restrict__ ranlux,
                                                           u32* __restrict__ carry, u32* __restrict__ pos_out,
                                                           u64* __restrict__ lcg) {
+  __shared__ uint4 stage[kRawStageWords];
   const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
-  if (i >= n) return;
-  u32 x[18], v[18], pos, c;
-  load_state(st, n, i, x, pos);
-  to_ranlux_exact(x, v, c);
+  const bool live = i < n;
+  u32 x[18], v[18], pos = 12, c = 0;
 #pragma unroll
-  for (int l = 0; l < 9; l++) {
-    if (ranlux) ranlux[i * 9 + l] = (u64)v[2 * l] | ((u64)v[2 * l + 1] << 32);
-    if (lcg) lcg[i * 9 + l] = (u64)x[2 * l] | ((u64)x[2 * l + 1] << 32);
+  for (int j = 0; j < 18; j++) { x[j] = 0; v[j] = 0; }
+  if (live) {
+    load_state(st, n, i, x, pos);
+    to_ranlux_exact(x, v, c);
   }
-  if (carry) carry[i] = c;
-  if (pos_out) pos_out[i] = pos;
+  if (ranlux) {  // uniform branches: the staged stores are CTA-collective
+    if (aligned16(ranlux)) store_raw<RLXPP_AOS>(ranlux, n, stage, v, blockIdx.x);
+    else if (live) store_u64x9(ranlux, i, v);
+  }
+  if (lcg) {
+    if (aligned16(lcg)) store_raw<RLXPP_AOS>(lcg, n, stage, x, blockIdx.x);
+    else if (live) store_u64x9(lcg, i, x);
+  }
+  if (live && carry) carry[i] = c;
+  if (live && pos_out) pos_out[i] = pos;
 }
 
 __global__ void __launch_bounds__(kThreads) import_kernel(uint4* __restrict__ st, u64 n, const u64* __restrict__ lcg,
                                                           const u32* __restrict__ pos_in) {
+  __shared__ uint4 stage[kRawStageWords];
   const u64 i = (u64)blockIdx.x * kThreads + threadIdx.x;
-  if (i >= n) return;
-  u32 z[20], x[18];
+  u32 w[18], z[20], x[18];
+  if (aligned16(lcg)) {
+    load_raw<RLXPP_AOS>(lcg, n, stage, w, blockIdx.x);
+  } else if (i < n) {
 #pragma unroll
-  for (int l = 0; l < 9; l++) {
-    const u64 w = lcg[i * 9 + l];
-    z[2 * l] = (u32)w;
-    z[2 * l + 1] = (u32)(w >> 32);
+    for (int l = 0; l < 9; l++) {
+      const u64 q = lcg[i * 9 + l];
+      w[2 * l] = (u32)q;
+      w[2 * l + 1] = (u32)(q >> 32);
+    }
   }
+  if (i >= n) return;
+#pragma unroll
+  for (int j = 0; j < 18; j++) z[j] = w[j];
   z[18] = 0; z[19] = 0;
   mod_m20(z, x);
   u32 pos = pos_in ? pos_in[i] : 12u;

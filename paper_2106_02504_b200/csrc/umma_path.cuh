@@ -33,7 +33,6 @@
 // profiles/ab_r02_pairs.md section 6.  GroupTile below still uses shared memory: six accumulators leave no columns.)
 #pragma once
 #include "arith.cuh"
-#include "umma.cuh"
 
 namespace rlx {
 namespace tc {

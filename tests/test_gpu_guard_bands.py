@@ -143,6 +143,22 @@ def test_raw_advance_and_state_export_stay_inside_their_buffers(rlx, torch, engi
         rlx.rlxpp_get_state(h, V.t, c.t.view(torch.int32), pos.t.view(torch.int32), X.t)
         for g, name in ((V, "ranlux"), (X, "lcg"), (c, "carry"), (pos, "cursor")):
             g.check(f"get_state {name}", full=False)
+        # arrays that are only 8-byte aligned take the per-thread path of the export / import kernels instead of the
+        # shared-memory stage: same contents, same bounds, and a handle loaded from them exports the same states
+        V8, X8 = Guarded(torch, 2701), Guarded(torch, 2701)
+        rlx.rlxpp_get_state(h, V8.t[1:], None, None, X8.t[1:])
+        V8.check("get_state ranlux, 8-byte aligned", full=False)
+        X8.check("get_state lcg, 8-byte aligned", full=False)
+        assert int(V8.t[0]) == int(SENTINEL) and int(X8.t[0]) == int(SENTINEL)
+        assert torch.equal(V8.t[1:], V.t) and torch.equal(X8.t[1:], X.t)
+        for src in (X.t, X8.t[1:]):
+            h2 = rlx.rlxpp_create(300, 1, 389)
+            rlx.rlxpp_set_state(h2, src, pos.t.view(torch.int32)[:300])
+            back = Guarded(torch, 2700)
+            rlx.rlxpp_get_state(h2, None, None, None, back.t)
+            back.check("set_state / get_state round trip", full=False)
+            assert torch.equal(back.t, X.t)
+            rlx.rlxpp_destroy(h2)
         rlx.rlxpp_destroy(h)
     finally:
         rlx.rlxpp_set_engine(rlx.RLXPP_ENGINE_UMMA)
